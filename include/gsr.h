@@ -1,0 +1,162 @@
+/*
+ * gsr.h -- C ABI of the B200-native AVU-GSR hot path (aprod1, aprod2, LSQR).
+ *
+ * The operations are the ones the paper states (arxiv 2503.22863, /root/reference/PAPER.md):
+ *   the system  A x = b                     PAPER.md:37   Sec. 2, Eq. (1)
+ *   the storage: <= 24 non-zeros per row,   PAPER.md:39   Sec. 2 (N_Astro=5, N_Att=12,
+ *                fp64                                      N_Instr=6, N_Glob=1)
+ *   aprod 1:  b^itn += A   x^(itn-1)        PAPER.md:45   Sec. 2, Eq. (2)
+ *   aprod 2:  x^itn += A^T b^itn            PAPER.md:49   Sec. 2, Eq. (3)
+ *   the LSQR loop around them               PAPER.md:53-64 Sec. 2 (steps 3-4), Sec. 2.1,
+ *                                           refs [29,30] (Paige & Saunders) PAPER.md:234-235
+ * The call list (gsr_create / gsr_aprod1 / gsr_aprod2 / gsr_lsqr) is the one named by
+ * BASELINE.json:north_star; the paper itself defines no API.
+ *
+ * DATA LAYOUT.  S stars, M rows, K attitude knots per axis, I instrumental
+ * parameters, G in {0,1} global parameters.
+ *   unknowns  x[n], n = 5S + 3K + I + G, blocks in the paper's order
+ *             [ astrometric 5S | attitude 3K (axis-major, axis offset K) | instrumental I | global G ]
+ *   values    M x 24 fp64, row-major: slots 0-4 astrometric, 5-16 attitude (axis a, knot j at
+ *             slot 5+4a+j), 17-22 instrumental, 23 global (ignored when G = 0)
+ *   indices   M x 8 int32, row-major: {star, att_start, instr_col[0..5]}
+ *   column of slot k of row r:
+ *             k < 5        : 5*star + k
+ *             5 <= k < 17  : 5S + a*K + att_start + j          (a = (k-5)/4, j = (k-5)%4)
+ *             17 <= k < 23 : 5S + 3K + instr_col[k-17]
+ *             k == 23      : 5S + 3K + I
+ *   Rows must be sorted by star (non-decreasing star id); this is validated.
+ *
+ * POINTERS.  Unless a parameter says "host", every array argument is a DEVICE pointer owned by
+ * the caller.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * All calls are for one GPU (the current device); there is no CPU fallback: without a CUDA
+ * device every call that would compute returns GSR_ECUDA.
+ *
+ * ERRORS.  Every int-returning call returns GSR_OK (0) or a negative code; nothing is printed,
+ * nothing throws, nothing exits.  gsr_strerror() names a code.
+ *
+ * DETERMINISM.  aprod2 uses fp64 reductions at L2 (red.global.add.f64) for the attitude block;
+ * the order of those additions varies run to run, so results are reproducible to rounding
+ * (normwise ~1e-15), not bit for bit.  aprod1 is bit-reproducible.
+ */
+#ifndef GSR_H
+#define GSR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSR_OK 0
+#define GSR_EINVAL (-1)  /* null pointer, bad size, n_glob not 0/1, misaligned pointer          */
+#define GSR_ELAYOUT (-2) /* index records violate the layout (star order/range, att_start, col) */
+#define GSR_ENOMEM (-3)  /* device or host allocation failed                                    */
+#define GSR_ECUDA (-4)   /* a CUDA call failed (sticky; see gsr_last_cuda_error)                */
+#define GSR_ESTATE (-5)  /* call out of order (e.g. iterate before init)                        */
+
+typedef struct gsr_system gsr_system; /* opaque */
+
+typedef struct {
+  int64_t n_rows;  /* M : observation rows + constraint rows            */
+  int64_t n_stars; /* S : astrometric block = 5*S columns                             */
+  int64_t n_knots; /* K : attitude block = 3*K columns, axis offset K; K >= 4         */
+  int64_t n_instr; /* I : instrumental block; I >= 1                                  */
+  int32_t n_glob;  /* G : 0 or 1 (the paper's tests use 0)              */
+  int32_t flags;   /* reserved, must be 0                                             */
+} gsr_layout;
+
+typedef struct {
+  int32_t istop; /* Paige-Saunders stop code 0..7 (not an error)                      */
+  int64_t itn;   /* iterations performed                                              */
+  double r1norm, r2norm; /* ||b - A x|| estimate (equal: damp = 0)                    */
+  double anorm, acond, arnorm, xnorm, bnorm;
+} gsr_lsqr_result;
+
+/* Scalars of the LSQR recurrences, as exported by gsr_lsqr_get_state (host struct). */
+typedef struct {
+  int64_t itn;
+  int32_t istop;
+  double alpha, beta, rhobar, phibar, bnorm, rnorm, arnorm, anorm, acond, ddnorm, xnorm, xxnorm,
+      z, cs2, sn2;
+} gsr_lsqr_scalars;
+
+/* ---- system -------------------------------------------------------------------------------
+ * gsr_create: bind a system to its device-resident matrix (PAPER.md:39 storage).
+ *   layout  : host pointer, copied.
+ *   values  : device, M*24 fp64, 32-byte aligned.  BORROWED, not copied (at 5e8 rows the matrix
+ *   indices : device, M*8 int32, 32-byte aligned.   is 112 GB): the caller keeps both alive and
+ *             unmodified until gsr_destroy.
+ *   Validates every index record on the device (GSR_ELAYOUT on violation), builds the side
+ *   structures (a few MB) and synchronises `stream` once.  M = 0 is allowed.
+ * gsr_destroy: frees everything the library allocated (never values/indices). NULL is a no-op. */
+int gsr_create(gsr_system **out, const gsr_layout *layout, const double *values,
+               const int32_t *indices, void *stream);
+void gsr_destroy(gsr_system *sys);
+int gsr_dims(const gsr_system *sys, int64_t *n_rows, int64_t *n_unknowns); /* host out-pointers */
+
+/* ---- the two products (asynchronous on `stream`) --------------------------------------------
+ * gsr_aprod1:  y[r] += sum_k a[r][k] * x[col(r,k)]      Eq. (2).  x: n, y: M.
+ * gsr_aprod2:  x[col(r,k)] += a[r][k] * y[r]            Eq. (3).  y: M, x: n.
+ * Both ACCUMULATE into their output (the paper's "+="); the input vector is not modified;
+ * input and output must not overlap.  Repeated instrumental columns inside a row accumulate. */
+int gsr_aprod1(gsr_system *sys, const double *x, double *y, void *stream);
+int gsr_aprod2(gsr_system *sys, const double *y, double *x, void *stream);
+
+/* ---- LSQR (Paige-Saunders, damp = 0) ---------------------------------
+ * gsr_lsqr: solve min ||A x - b||_2 from x = 0.
+ *   b (device, M) is not modified; x (device, n) is overwritten with the solution.
+ *   itnlim >= 0; atol, btol >= 0; conlim >= 0 (0 = no condition-number test).
+ *   res (HOST pointer) receives istop, itn and the norm estimates.
+ *   Returns after the result is on the host (synchronises `stream`).
+ *   istop: 0 x=0 is exact; 1 Ax=b to atol/btol; 2 least-squares solution to atol; 3 acond >=
+ *   conlim; 4,5,6 the same three at machine precision; 7 itnlim reached.
+ * Work vectors (u: M; v, w, x: n) are allocated on the first call and reused.
+ *
+ * The same solve, in steps (used by the benchmark to time exactly K iterations and by the
+ * parity tests to compare one iteration at a time):
+ *   gsr_lsqr_init    : x = 0; beta u = b; alpha v = A^T u; w = v     ("initial
+ *                      conditions are set with aprod 2").  Asynchronous.
+ *   gsr_lsqr_iterate : up to n_iters further iterations (each: aprod 1, aprod 2, the vector
+ *                      updates, norms and stopping tests, all on the device); iterations after
+ *                      a stop (istop != 0) are no-ops.  Asynchronous; the stopping rule is
+ *                      evaluated on the device with the given tolerances.
+ *   gsr_lsqr_result_get : copy the solution into x_out (device, n; may be NULL) and fill *res
+ *                      (host).  Synchronises `stream`.
+ *   gsr_lsqr_get_state : export the normalised Golub-Kahan vectors u (M), v, w, x (n) (device
+ *                      pointers, any may be NULL) and the scalars (host).  Synchronises.      */
+int gsr_lsqr(gsr_system *sys, const double *b, double *x, int64_t itnlim, double atol,
+             double btol, double conlim, gsr_lsqr_result *res, void *stream);
+int gsr_lsqr_init(gsr_system *sys, const double *b, void *stream);
+int gsr_lsqr_iterate(gsr_system *sys, int64_t n_iters, int64_t itnlim, double atol, double btol,
+                     double conlim, void *stream);
+int gsr_lsqr_result_get(gsr_system *sys, double *x_out, gsr_lsqr_result *res, void *stream);
+int gsr_lsqr_get_state(gsr_system *sys, double *u, double *v, double *w, double *x,
+                       gsr_lsqr_scalars *scalars, void *stream);
+
+/* ---- whole solve from HOST buffers (end-to-end path) ----------------------------------------
+ * Allocates device memory, copies values / indices / b host->device, runs gsr_create + gsr_lsqr,
+ * copies x device->host, frees everything.  All four arrays are HOST pointers (pinned or
+ * pageable); x_host (n) is overwritten.  Blocking. */
+int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int32_t *indices_host,
+                  const double *b_host, double *x_host, int64_t itnlim, double atol, double btol,
+                  double conlim, gsr_lsqr_result *res);
+
+/* ---- diagnostics ----------------------------------------------------------------------------
+ * gsr_launch_count : kernels launched by this system object so far (host out-pointer).
+ * gsr_profile      : enable (1) / disable (0) CUDA-event timing of the aprod1 / aprod2 kernels
+ *                    issued by gsr_lsqr_iterate and gsr_aprod1/2 on their own stream.
+ * gsr_profile_get  : after a synchronise, mean duration in ms and launch count since the last
+ *                    call, per kernel class: which = 1 aprod1, 2 aprod2 (host out-pointers).
+ * gsr_set_option   : tuning knobs; unknown names -> GSR_EINVAL.          */
+int gsr_launch_count(const gsr_system *sys, int64_t *n_launches);
+int gsr_profile(gsr_system *sys, int enable);
+int gsr_profile_get(gsr_system *sys, int which, double *mean_ms, int64_t *count);
+int gsr_set_option(gsr_system *sys, const char *name, int64_t value);
+const char *gsr_strerror(int code);
+const char *gsr_last_cuda_error(void); /* text of the last CUDA failure in this thread, or "" */
+const char *gsr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSR_H */

@@ -1,0 +1,387 @@
+// C ABI of libgsr (include/gsr.h): argument checking, ownership, the LSQR driver.
+// Every step of the path runs in the kernels of aprod1.cu / aprod2.cu / lsqr_kernels.cu.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gsr_internal.cuh"
+
+using namespace gsr;
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+  return GSR_ECUDA;
+}
+#define CU(call)                                           \
+  do {                                                     \
+    cudaError_t e_ = (call);                               \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);    \
+  } while (0)
+
+struct EventPair {
+  cudaEvent_t a, b;
+  int which;
+};
+
+struct gsr_system {
+  SysView v;
+  Tuning tune;
+  int device = 0;
+  int num_sms = 148;
+  int64_t launches = 0;
+  // LSQR workspace (allocated on first use)
+  double *u = nullptr, *vv = nullptr, *w = nullptr, *x = nullptr;
+  DevScalars* sc = nullptr;
+  bool lsqr_ready = false;   // gsr_lsqr_init has run
+  // profiling
+  bool profile = false;
+  std::vector<EventPair> pending;
+  std::vector<EventPair> pool;
+  double prof_ms[3] = {0, 0, 0};
+  int64_t prof_n[3] = {0, 0, 0};
+};
+
+static inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+extern "C" const char* gsr_strerror(int code) {
+  switch (code) {
+    case GSR_OK: return "ok";
+    case GSR_EINVAL: return "invalid argument";
+    case GSR_ELAYOUT: return "index records violate the layout";
+    case GSR_ENOMEM: return "out of memory";
+    case GSR_ECUDA: return "CUDA error";
+    case GSR_ESTATE: return "call out of order";
+    default: return "unknown error";
+  }
+}
+extern "C" const char* gsr_last_cuda_error(void) { return g_cuda_err; }
+extern "C" const char* gsr_version(void) { return "gsr-b200 0.1 (sm_100a)"; }
+
+static bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* values,
+                          const int32_t* indices, void* stream) {
+  if (!out) return GSR_EINVAL;
+  *out = nullptr;
+  if (!L) return GSR_EINVAL;
+  if (L->n_rows < 0 || L->n_stars < 1 || L->n_knots < 4 || L->n_instr < 1) return GSR_EINVAL;
+  if (L->n_glob != 0 && L->n_glob != 1) return GSR_EINVAL;
+  if (L->flags != 0) return GSR_EINVAL;
+  if (L->n_stars > INT32_MAX || L->n_knots > INT32_MAX || L->n_instr > INT32_MAX) return GSR_EINVAL;
+  if (L->n_rows > 0 && (!values || !indices)) return GSR_EINVAL;
+  if (!aligned(values, 32) || !aligned(indices, 32)) return GSR_EINVAL;
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  gsr_system* s = new (std::nothrow) gsr_system();
+  if (!s) return GSR_ENOMEM;
+  s->device = dev;
+  cudaError_t e = cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaDeviceGetAttribute"); }
+  SysView& v = s->v;
+  v.vals = values; v.idx = indices;
+  v.M = L->n_rows; v.S = L->n_stars; v.K = L->n_knots; v.I = L->n_instr; v.G = L->n_glob;
+  v.oA = 5 * v.S; v.oI = v.oA + 3 * v.K; v.oG = v.oI + v.I; v.n = v.oG + v.G;
+  // device-side validation of every index record
+  int* flag = nullptr;
+  e = cudaMalloc(&flag, sizeof(int));
+  if (e != cudaSuccess) { delete s; return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc"); }
+  int h = 0;
+  cudaStream_t st = S(stream);
+  e = cudaMemsetAsync(flag, 0, sizeof(int), st);
+  if (e == cudaSuccess) e = launch_validate(v, flag, st, &s->launches);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(flag);
+  if (e != cudaSuccess) { delete s; return cuda_fail(e, "gsr_create validation"); }
+  if (h != 0) { delete s; return GSR_ELAYOUT; }
+  *out = s;
+  return GSR_OK;
+}
+
+static void free_events(gsr_system* s) {
+  for (auto& p : s->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+  for (auto& p : s->pool) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+  s->pending.clear();
+  s->pool.clear();
+}
+
+extern "C" void gsr_destroy(gsr_system* s) {
+  if (!s) return;
+  cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
+  free_events(s);
+  delete s;
+}
+
+extern "C" int gsr_dims(const gsr_system* s, int64_t* m, int64_t* n) {
+  if (!s) return GSR_EINVAL;
+  if (m) *m = s->v.M;
+  if (n) *n = s->v.n;
+  return GSR_OK;
+}
+
+// ---- profiling helpers ---------------------------------------------------------------------
+static bool prof_begin(gsr_system* s, int which, cudaStream_t st, EventPair* ep) {
+  if (!s->profile) return false;
+  if (!s->pool.empty()) { *ep = s->pool.back(); s->pool.pop_back(); }
+  else {
+    if (cudaEventCreate(&ep->a) != cudaSuccess) return false;
+    if (cudaEventCreate(&ep->b) != cudaSuccess) { cudaEventDestroy(ep->a); return false; }
+  }
+  ep->which = which;
+  cudaEventRecord(ep->a, st);
+  return true;
+}
+static void prof_end(gsr_system* s, cudaStream_t st, EventPair* ep) {
+  cudaEventRecord(ep->b, st);
+  s->pending.push_back(*ep);
+}
+
+static int do_aprod1(gsr_system* s, const double* x, double* y, const double* c0, double* sumsq,
+                     int* done, cudaStream_t st) {
+  EventPair ep;
+  const bool p = prof_begin(s, 1, st, &ep);
+  cudaError_t e = launch_aprod1(s->v, s->tune, s->num_sms, x, y, c0, sumsq, done, st, &s->launches);
+  if (p) prof_end(s, st, &ep);
+  if (e != cudaSuccess) return cuda_fail(e, "aprod1 launch");
+  return GSR_OK;
+}
+static int do_aprod2(gsr_system* s, const double* y, double* x, const double* yscale, const int* done,
+                     cudaStream_t st) {
+  EventPair ep;
+  const bool p = prof_begin(s, 2, st, &ep);
+  cudaError_t e = launch_aprod2(s->v, s->tune, s->num_sms, y, x, yscale, done, st, &s->launches);
+  if (p) prof_end(s, st, &ep);
+  if (e != cudaSuccess) return cuda_fail(e, "aprod2 launch");
+  return GSR_OK;
+}
+
+extern "C" int gsr_aprod1(gsr_system* s, const double* x, double* y, void* stream) {
+  if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
+  return do_aprod1(s, x, y, nullptr, nullptr, nullptr, S(stream));
+}
+extern "C" int gsr_aprod2(gsr_system* s, const double* y, double* x, void* stream) {
+  if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
+  return do_aprod2(s, y, x, nullptr, nullptr, S(stream));
+}
+
+// ---- LSQR ------------------------------------------------------------------------------------
+static int ensure_workspace(gsr_system* s) {
+  if (s->sc) return GSR_OK;
+  const size_t m = (size_t)(s->v.M > 0 ? s->v.M : 1), n = (size_t)s->v.n;
+  cudaError_t e;
+  if ((e = cudaMalloc(&s->u, m * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->vv, n * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->w, n * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->x, n * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->sc, sizeof(DevScalars))) != cudaSuccess) {
+    cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
+    s->u = s->vv = s->w = s->x = nullptr; s->sc = nullptr;
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc workspace");
+  }
+  return GSR_OK;
+}
+
+extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
+  if (!s || (!b && s->v.M > 0)) return GSR_EINVAL;
+  int rc = ensure_workspace(s);
+  if (rc) return rc;
+  cudaStream_t st = S(stream);
+  const int64_t M = s->v.M, n = s->v.n;
+  CU(cudaMemsetAsync(s->sc, 0, sizeof(DevScalars), st));
+  CU(cudaMemsetAsync(s->vv, 0, (size_t)n * sizeof(double), st));
+  CU(lsqr_launch_init_u(b, s->u, M, s->sc, st, &s->launches));           // u_hat = b, usq
+  CU(lsqr_launch_init_s1(s->sc, st, &s->launches));                      // beta
+  rc = do_aprod2(s, s->u, s->vv, &s->sc->s_y, nullptr, st);              // v = A^T u
+  if (rc) return rc;
+  CU(lsqr_launch_sumsq_v(s->vv, n, s->sc, st, &s->launches));
+  CU(lsqr_launch_init_s2(s->sc, st, &s->launches));                      // alpha and the rest
+  CU(lsqr_launch_init_vw(s->vv, s->w, s->x, n, s->sc, st, &s->launches));
+  s->lsqr_ready = true;
+  return GSR_OK;
+}
+
+extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, double atol, double btol,
+                                double conlim, void* stream) {
+  if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
+  if (!s->lsqr_ready) return GSR_ESTATE;
+  cudaStream_t st = S(stream);
+  const int64_t n = s->v.n;
+  DevScalars* sc = s->sc;
+  for (int64_t it = 0; it < n_iters; ++it) {
+    // 1: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2              (aprod 1)
+    int rc = do_aprod1(s, s->vv, s->u, &sc->c0_u, &sc->usq, &sc->done, st);
+    if (rc) return rc;
+    // 2: beta ; v <- -beta v ; v += A^T (u_hat / beta) ; vsq = ||v||^2      (aprod 2)
+    CU(lsqr_launch_vscale(s->vv, n, sc, st, &s->launches));
+    rc = do_aprod2(s, s->u, s->vv, &sc->s_y, &sc->done, st);
+    if (rc) return rc;
+    CU(lsqr_launch_sumsq_v(s->vv, n, sc, st, &s->launches));
+    // 3-8: scalars, stopping rule ; then the x / w / v update
+    CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
+    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, st, &s->launches));
+  }
+  return GSR_OK;
+}
+
+static int fetch_scalars(gsr_system* s, DevScalars* h, cudaStream_t st) {
+  CU(cudaMemcpyAsync(h, s->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return GSR_OK;
+}
+
+static void fill_result(const DevScalars& h, gsr_lsqr_result* res) {
+  res->istop = h.istop; res->itn = h.itn;
+  res->r1norm = h.rnorm; res->r2norm = h.rnorm;
+  res->anorm = h.anorm; res->acond = h.acond; res->arnorm = h.arnorm;
+  res->xnorm = h.xnorm; res->bnorm = h.bnorm;
+}
+
+extern "C" int gsr_lsqr_result_get(gsr_system* s, double* x_out, gsr_lsqr_result* res, void* stream) {
+  if (!s || !res) return GSR_EINVAL;
+  if (!s->lsqr_ready) return GSR_ESTATE;
+  cudaStream_t st = S(stream);
+  if (x_out) CU(cudaMemcpyAsync(x_out, s->x, (size_t)s->v.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  DevScalars h;
+  int rc = fetch_scalars(s, &h, st);
+  if (rc) return rc;
+  fill_result(h, res);
+  return GSR_OK;
+}
+
+extern "C" int gsr_lsqr_get_state(gsr_system* s, double* u, double* v, double* w, double* x,
+                                  gsr_lsqr_scalars* out, void* stream) {
+  if (!s) return GSR_EINVAL;
+  if (!s->lsqr_ready) return GSR_ESTATE;
+  cudaStream_t st = S(stream);
+  const size_t nb = (size_t)s->v.n * sizeof(double);
+  if (u && s->v.M > 0) CU(lsqr_launch_export_u(s->u, u, s->v.M, s->sc, st, &s->launches));
+  if (v) CU(cudaMemcpyAsync(v, s->vv, nb, cudaMemcpyDeviceToDevice, st));
+  if (w) CU(cudaMemcpyAsync(w, s->w, nb, cudaMemcpyDeviceToDevice, st));
+  if (x) CU(cudaMemcpyAsync(x, s->x, nb, cudaMemcpyDeviceToDevice, st));
+  DevScalars h;
+  int rc = fetch_scalars(s, &h, st);
+  if (rc) return rc;
+  if (out) {
+    out->itn = h.itn; out->istop = h.istop;
+    out->alpha = h.alpha; out->beta = h.beta; out->rhobar = h.rhobar; out->phibar = h.phibar;
+    out->bnorm = h.bnorm; out->rnorm = h.rnorm; out->arnorm = h.arnorm; out->anorm = h.anorm;
+    out->acond = h.acond; out->ddnorm = h.ddnorm; out->xnorm = h.xnorm; out->xxnorm = h.xxnorm;
+    out->z = h.z; out->cs2 = h.cs2; out->sn2 = h.sn2;
+  }
+  return GSR_OK;
+}
+
+extern "C" int gsr_lsqr(gsr_system* s, const double* b, double* x, int64_t itnlim, double atol,
+                        double btol, double conlim, gsr_lsqr_result* res, void* stream) {
+  if (!s || !x || !res || itnlim < 0) return GSR_EINVAL;
+  int rc = gsr_lsqr_init(s, b, stream);
+  if (rc) return rc;
+  cudaStream_t st = S(stream);
+  DevScalars h;
+  if ((rc = fetch_scalars(s, &h, st))) return rc;
+  if (!h.done && itnlim == 0) {
+    h.istop = 7;
+    CU(cudaMemcpyAsync(&s->sc->istop, &h.istop, sizeof(int), cudaMemcpyHostToDevice, st));
+  }
+  int64_t issued = 0;
+  while (!h.done && issued < itnlim) {
+    int64_t batch = s->tune.check_every > 0 ? s->tune.check_every : 16;
+    if (batch > itnlim - issued) batch = itnlim - issued;
+    if ((rc = gsr_lsqr_iterate(s, batch, itnlim, atol, btol, conlim, stream))) return rc;
+    issued += batch;
+    if ((rc = fetch_scalars(s, &h, st))) return rc;   // poll the device-side stop flag
+  }
+  return gsr_lsqr_result_get(s, x, res, stream);
+}
+
+extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, const int32_t* indices_host,
+                             const double* b_host, double* x_host, int64_t itnlim, double atol, double btol,
+                             double conlim, gsr_lsqr_result* res) {
+  if (!L || !x_host || !res || L->n_rows < 0) return GSR_EINVAL;
+  if (L->n_rows > 0 && (!values_host || !indices_host || !b_host)) return GSR_EINVAL;
+  const size_t M = (size_t)L->n_rows;
+  const size_t n = (size_t)(5 * L->n_stars + 3 * L->n_knots + L->n_instr + L->n_glob);
+  double *dv = nullptr, *db = nullptr, *dx = nullptr;
+  int32_t* di = nullptr;
+  gsr_system* sys = nullptr;
+  cudaStream_t st = nullptr;
+  int rc = GSR_OK;
+  cudaError_t e;
+  auto cleanup = [&]() {
+    gsr_destroy(sys);
+    cudaFree(dv); cudaFree(di); cudaFree(db); cudaFree(dx);
+    if (st) cudaStreamDestroy(st);
+  };
+  if ((e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+  if ((e = cudaMalloc(&dv, (M ? M : 1) * NSLOT * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&di, (M ? M : 1) * NIDX * sizeof(int32_t))) != cudaSuccess ||
+      (e = cudaMalloc(&db, (M ? M : 1) * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&dx, n * sizeof(double))) != cudaSuccess) {
+    cleanup();
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc");
+  }
+  if (M) {
+    if ((e = cudaMemcpyAsync(di, indices_host, M * NIDX * sizeof(int32_t), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dv, values_host, M * NSLOT * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(db, b_host, M * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+      cleanup();
+      return cuda_fail(e, "cudaMemcpyAsync H2D");
+    }
+  }
+  rc = gsr_create(&sys, L, dv, di, st);
+  if (rc == GSR_OK) rc = gsr_lsqr(sys, db, dx, itnlim, atol, btol, conlim, res, st);
+  if (rc == GSR_OK) {
+    e = cudaMemcpyAsync(x_host, dx, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "cudaMemcpyAsync D2H");
+  }
+  cleanup();
+  return rc;
+}
+
+// ---- diagnostics ---------------------------------------------------------------------------
+extern "C" int gsr_launch_count(const gsr_system* s, int64_t* n) {
+  if (!s || !n) return GSR_EINVAL;
+  *n = s->launches;
+  return GSR_OK;
+}
+
+extern "C" int gsr_profile(gsr_system* s, int enable) {
+  if (!s) return GSR_EINVAL;
+  s->profile = enable != 0;
+  return GSR_OK;
+}
+
+extern "C" int gsr_profile_get(gsr_system* s, int which, double* mean_ms, int64_t* count) {
+  if (!s || which < 1 || which > 2) return GSR_EINVAL;
+  for (auto& p : s->pending) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(p.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaEventElapsedTime");
+    s->prof_ms[p.which] += ms;
+    s->prof_n[p.which] += 1;
+    s->pool.push_back(p);
+  }
+  s->pending.clear();
+  if (mean_ms) *mean_ms = s->prof_n[which] ? s->prof_ms[which] / (double)s->prof_n[which] : 0.0;
+  if (count) *count = s->prof_n[which];
+  s->prof_ms[which] = 0.0;
+  s->prof_n[which] = 0;
+  return GSR_OK;
+}
+
+extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
+  if (!s || !name) return GSR_EINVAL;
+  if (!strcmp(name, "aprod1_variant")) s->tune.aprod1_variant = (int)value;
+  else if (!strcmp(name, "aprod2_variant")) s->tune.aprod2_variant = (int)value;
+  else if (!strcmp(name, "ctas_per_sm")) s->tune.ctas_per_sm = (int)value;
+  else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;
+  else return GSR_EINVAL;
+  return GSR_OK;
+}

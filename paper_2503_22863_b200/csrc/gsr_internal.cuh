@@ -1,0 +1,84 @@
+// Internal declarations of libgsr (not part of the ABI; the ABI is include/gsr.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gsr.h"
+
+namespace gsr {
+
+constexpr int NSLOT = 24;  // PAPER.md:39 : 5 astro + 12 attitude + 6 instrumental + 1 global
+constexpr int NIDX = 8;    // {star, att_start, instr[6]}
+
+// Read-only view of a system, passed by value to kernels.
+struct SysView {
+  const double* vals;   // M x 24
+  const int32_t* idx;   // M x 8
+  int64_t M, S, K, I;
+  int32_t G;
+  int64_t oA, oI, oG, n;  // block offsets in x: attitude, instrumental, global; n unknowns
+};
+
+// Device-resident LSQR scalars.  One instance per system.
+struct DevScalars {
+  double alpha, beta, rhobar, phibar, bnorm, rnorm, arnorm, anorm, acond, ddnorm, xnorm, xxnorm,
+      z, cs2, sn2;
+  double usq, vsq, wsq;          // sum-of-squares accumulators (atomically added by kernels)
+  double c0_u;                   // aprod1 fused update: u_hat <- A v + c0_u * u_hat  (= -alpha/beta)
+  double s_y;                    // aprod2 input scale (1/beta: u = u_hat / beta is never stored)
+  double t1, t2, inv_alpha;      // x/w/v update coefficients of the current iteration
+  long long itn;
+  int istop;
+  int done;                      // 1 once a stopping rule fired: later kernels are no-ops
+};
+
+struct Tuning {
+  int aprod1_variant = 0;
+  int aprod2_variant = 0;
+  int ctas_per_sm = 0;  // 0 = default of the variant
+  int check_every = 16; // LSQR iterations between host polls of the stop flag
+};
+
+// Launchers (each returns cudaGetLastError()).  Null coefficient pointers mean 1.0 / "no".
+//   aprod1: y[r] = c1 * (A x)[r] + c0 * y[r]      (c0 = c1 = 1 -> Eq. 2);  *sumsq += sum y[r]^2
+cudaError_t launch_aprod1(const SysView& s, const Tuning& t, int num_sms, const double* x, double* y,
+                          const double* c0, double* sumsq, int* done, cudaStream_t st,
+                          int64_t* launches);
+//   aprod2: x += A^T (yscale * y)
+cudaError_t launch_aprod2(const SysView& s, const Tuning& t, int num_sms, const double* y, double* x,
+                          const double* yscale, const int* done, cudaStream_t st, int64_t* launches);
+cudaError_t launch_validate(const SysView& s, int* flag, cudaStream_t st, int64_t* launches);
+
+// LSQR vector / scalar kernels (lsqr_kernels.cu)
+cudaError_t lsqr_launch_init_u(const double* b, double* u, int64_t M, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_sumsq_v(const double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
+                                     cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches);
+
+// ---- device helpers -----------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Block-wide sum (blockDim.x multiple of 32, <= 1024); result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v) {
+  __shared__ double part[32];
+  v = warp_sum(v);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) part[w] = v;
+  __syncthreads();
+  const int nw = (blockDim.x + 31) >> 5;
+  v = (threadIdx.x < nw) ? part[threadIdx.x] : 0.0;
+  if (w == 0) v = warp_sum(v);
+  return v;
+}
+
+}  // namespace gsr

@@ -1,0 +1,237 @@
+// LSQR vector updates, norms, scalar recurrences and stopping tests, all on the device
+// (Paige-Saunders LSQR, paper refs [29,30]; solver outline PAPER.md:53-64;
+// SURVEY.md section 8a rows a6-a10).
+//
+// u is kept UN-normalised (u_hat = beta * u): the scale 1/beta is applied by the consumer
+// (aprod2 reads yscale = 1/beta), so no M-length scale pass exists.  v, w, x are n-length
+// (n << M) and are kept in the textbook (normalised) form.
+#include "gsr_internal.cuh"
+
+namespace gsr {
+
+static inline unsigned grid_for(int64_t n, int threads, int per_thread) {
+  int64_t b = (n + (int64_t)threads * per_thread - 1) / ((int64_t)threads * per_thread);
+  if (b < 1) b = 1;
+  if (b > 148 * 8) b = 148 * 8;
+  return (unsigned)b;
+}
+
+// u_hat = b ; usq = sum b^2                                                       (init)
+__global__ void __launch_bounds__(256) k_init_u(const double* __restrict__ b, double* __restrict__ u,
+                                                int64_t M, DevScalars* sc) {
+  double sq = 0.0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < M;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const double t = b[i];
+    u[i] = t;
+    sq = fma(t, t, sq);
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(&sc->usq, sq);
+}
+
+// beta = ||b||                                                                      (init)
+__global__ void k_init_s1(DevScalars* sc) {
+  const double beta = sqrt(sc->usq);
+  sc->beta = beta;
+  sc->bnorm = beta;
+  sc->s_y = beta > 0.0 ? 1.0 / beta : 0.0;
+  sc->usq = 0.0;
+  sc->vsq = 0.0;
+  sc->wsq = 0.0;
+  sc->done = 0;
+  sc->istop = 0;
+  sc->itn = 0;
+}
+
+__global__ void __launch_bounds__(256) k_sumsq_v(const double* __restrict__ v, int64_t n, DevScalars* sc) {
+  if (sc->done) return;
+  double sq = 0.0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const double t = v[i];
+    sq = fma(t, t, sq);
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(&sc->vsq, sq);
+}
+
+// alpha = ||A^T u||; the remaining initial scalars                                   (init)
+__global__ void k_init_s2(DevScalars* sc) {
+  const double beta = sc->beta;
+  const double alpha = beta > 0.0 ? sqrt(sc->vsq) : 0.0;
+  sc->alpha = alpha;
+  sc->inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
+  sc->arnorm = alpha * beta;
+  sc->rhobar = alpha;
+  sc->phibar = beta;
+  sc->rnorm = beta;
+  sc->anorm = 0.0; sc->acond = 0.0; sc->ddnorm = 0.0; sc->xnorm = 0.0; sc->xxnorm = 0.0;
+  sc->z = 0.0; sc->cs2 = -1.0; sc->sn2 = 0.0;
+  sc->c0_u = beta > 0.0 ? -alpha / beta : 0.0;
+  sc->vsq = 0.0;
+  if (alpha * beta == 0.0) { sc->istop = 0; sc->done = 1; }   // x = 0 is the exact solution
+}
+
+// v /= alpha ; w = v ; x = 0 ; wsq = ||w||^2                                         (init)
+__global__ void __launch_bounds__(256) k_init_vw(double* __restrict__ v, double* __restrict__ w,
+                                                 double* __restrict__ x, int64_t n, DevScalars* sc) {
+  const double ia = sc->inv_alpha;
+  double sq = 0.0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const double t = v[i] * ia;
+    v[i] = t;
+    w[i] = t;
+    x[i] = 0.0;
+    sq = fma(t, t, sq);
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(&sc->wsq, sq);
+}
+
+// step 2a: beta = ||u_hat||; v <- -beta v (then aprod2 adds A^T u).  Thread 0 publishes beta,
+// 1/beta and anorm; usq is left intact for the other blocks and cleared by k_step_scalars.
+__global__ void __launch_bounds__(256) k_vscale(double* __restrict__ v, int64_t n, DevScalars* sc) {
+  if (sc->done) return;
+  const double beta = sqrt(sc->usq);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    sc->beta = beta;
+    sc->s_y = beta > 0.0 ? 1.0 / beta : 0.0;
+    if (beta > 0.0) sc->anorm = sqrt(sc->anorm * sc->anorm + sc->alpha * sc->alpha + beta * beta);
+  }
+  if (!(beta > 0.0)) return;                         // P-S: v, alpha unchanged when beta = 0
+  const double nb = -beta;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    v[i] *= nb;
+}
+
+// steps 2b-8 of DESIGN.md section 4 (scalars only): alpha, plane rotation, norm estimates, stopping rule
+__global__ void k_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim) {
+  if (sc->done) return;
+  const double beta = sc->beta;
+  double alpha = sc->alpha;
+  if (beta > 0.0) alpha = sqrt(sc->vsq);
+  sc->inv_alpha = (beta > 0.0 && alpha > 0.0) ? 1.0 / alpha : 1.0;
+  // 3: plane rotation
+  const double rho = sqrt(sc->rhobar * sc->rhobar + beta * beta);
+  const double cs = sc->rhobar / rho, sn = beta / rho;
+  const double theta = sn * alpha;
+  sc->rhobar = -cs * alpha;
+  const double phi = cs * sc->phibar;
+  sc->phibar = sn * sc->phibar;
+  const double tau = sn * phi;
+  // 4: coefficients of the x / w update; ||w/rho||^2 = wsq / rho^2
+  sc->t1 = phi / rho;
+  sc->t2 = -theta / rho;
+  sc->ddnorm += sc->wsq / (rho * rho);
+  // 5: ||x|| estimate
+  const double delta = sc->sn2 * rho, gambar = -sc->cs2 * rho, rhs = phi - delta * sc->z;
+  const double zbar = rhs / gambar;
+  sc->xnorm = sqrt(sc->xxnorm + zbar * zbar);
+  const double gamma = sqrt(gambar * gambar + theta * theta);
+  sc->cs2 = gambar / gamma;
+  sc->sn2 = theta / gamma;
+  sc->z = rhs / gamma;
+  sc->xxnorm += sc->z * sc->z;
+  // 6: norm estimates
+  sc->acond = sc->anorm * sqrt(sc->ddnorm);
+  sc->rnorm = fabs(sc->phibar);
+  sc->arnorm = alpha * fabs(tau);
+  sc->alpha = alpha;
+  sc->c0_u = beta > 0.0 ? -alpha / beta : 0.0;      // next aprod1: u_hat <- A v - (alpha/beta) u_hat
+  const long long itn = ++sc->itn;
+  // 7-8: stopping rule (later tests override earlier ones)
+  const double ctol = conlim > 0.0 ? 1.0 / conlim : 0.0;
+  const double test1 = sc->rnorm / sc->bnorm;
+  const double den2 = sc->anorm * sc->rnorm;
+  const double test2 = den2 > 0.0 ? sc->arnorm / den2 : 0.0;
+  const double test3 = 1.0 / sc->acond;
+  const double t1p = test1 / (1.0 + sc->anorm * sc->xnorm / sc->bnorm);
+  const double rtol = btol + atol * sc->anorm * sc->xnorm / sc->bnorm;
+  int istop = 0;
+  if (itn >= itnlim) istop = 7;
+  if (1.0 + test3 <= 1.0) istop = 6;
+  if (1.0 + test2 <= 1.0) istop = 5;
+  if (1.0 + t1p <= 1.0) istop = 4;
+  if (test3 <= ctol) istop = 3;
+  if (test2 <= atol) istop = 2;
+  if (test1 <= rtol) istop = 1;
+  sc->istop = istop;
+  sc->usq = 0.0;
+  sc->vsq = 0.0;
+  sc->wsq = 0.0;
+  if (istop) sc->done = 2;  // 2 = stopped, but this iteration's k_update must still run (P-S updates x
+                            // before testing); the next aprod1 launch latches 2 -> 1
+}
+
+// step 4 (vectors): v /= alpha ; x += t1 w ; w = v + t2 w ; wsq = ||w_new||^2
+__global__ void __launch_bounds__(256) k_update(double* __restrict__ v, double* __restrict__ w,
+                                                double* __restrict__ x, int64_t n, DevScalars* sc) {
+  if (sc->done == 1) return;
+  const double ia = sc->inv_alpha, t1 = sc->t1, t2 = sc->t2;
+  double sq = 0.0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const double vi = v[i] * ia, wi = w[i];
+    v[i] = vi;
+    x[i] = fma(t1, wi, x[i]);
+    const double wn = fma(t2, wi, vi);
+    w[i] = wn;
+    sq = fma(wn, wn, sq);
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(&sc->wsq, sq);
+}
+
+// u = u_hat / beta (export only)
+__global__ void __launch_bounds__(256) k_export_u(const double* __restrict__ uhat, double* __restrict__ u,
+                                                  int64_t M, const DevScalars* sc) {
+  const double s = sc->s_y;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < M;
+       i += (int64_t)gridDim.x * blockDim.x)
+    u[i] = uhat[i] * s;
+}
+
+#define LAUNCHED() (++*launches, cudaGetLastError())
+
+cudaError_t lsqr_launch_init_u(const double* b, double* u, int64_t M, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_init_u<<<grid_for(M, 256, 4), 256, 0, st>>>(b, u, M, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_init_s1<<<1, 1, 0, st>>>(sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_sumsq_v(const double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_sumsq_v<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_init_s2<<<1, 1, 0, st>>>(sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_init_vw<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_vscale<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
+                                     cudaStream_t st, int64_t* launches) {
+  k_step_scalars<<<1, 1, 0, st>>>(sc, itnlim, atol, btol, conlim);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_update<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_export_u<<<grid_for(M, 256, 4), 256, 0, st>>>(uhat, u, M, sc);
+  return LAUNCHED();
+}
+
+}  // namespace gsr

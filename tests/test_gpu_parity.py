@@ -1,0 +1,401 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Run with -m gpu on the B200 box.
+
+Tolerances (BASELINE.json north_star):
+  aprod1  |y_gpu - y_ref| <= 1e-13 * (|y_in| + sum_k |a_k x_k|)    per row (reading R14)
+  aprod2  ||x_gpu - x_ref||_2 <= 1e-11 * ||x_ref||_2, overall and per block (reading R15)
+  LSQR    ||x_gpu - x_cpu|| <= 1e-9 ||x_cpu|| at the same iteration count where that is
+          well-posed (first iterations; at convergence), plus one-iteration replays from a
+          shared state for every sampled k (reading R16).
+"""
+import copy
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+import paper_2503_22863_b200 as gsr  # noqa: E402
+from gaia_synth import device as gdev  # noqa: E402
+from gaia_synth import host  # noqa: E402
+from gaia_synth.configs import C1, C2, C3, C5, SystemShape  # noqa: E402
+from helpers import nonempty_columns, rhs, tiny_shape  # noqa: E402
+
+DEV = "cuda"
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
+
+
+def make_gpu_system(shape, a, idx):
+    return gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, dev(a), dev(idx))
+
+
+def blocks_of(shape):
+    return {"astro": slice(0, shape.off_att), "att": slice(shape.off_att, shape.off_instr),
+            "instr": slice(shape.off_instr, shape.off_glob),
+            "glob": slice(shape.off_glob, shape.n_unknowns)}
+
+
+def check_aprod1(shape, a, idx, sys_, seed=1, y_in=None, threads=1):
+    L = oracle.layout_of(shape)
+    m, n = a.shape[0], shape.n_unknowns
+    x = host.test_vector(seed, 1, n)
+    y0 = host.test_vector(seed, 2, m) if y_in is None else y_in
+    ref = oracle.aprod1(L, a, idx, x, y0.copy(), threads=threads)
+    bound = oracle.aprod1_abs(L, a, idx, x, y0)
+    yg = dev(y0)
+    gsr.gsr_aprod1(sys_, dev(x), yg)
+    got = yg.cpu().numpy()
+    err = np.abs(got - ref)
+    assert np.all(err <= 1e-13 * bound), f"aprod1: max scaled err {np.max(err / np.maximum(bound, 1e-300)):.3e}"
+    return got
+
+
+def check_aprod2(shape, a, idx, sys_, seed=2, threads=1, x_in=None):
+    L = oracle.layout_of(shape)
+    m, n = a.shape[0], shape.n_unknowns
+    y = host.test_vector(seed, 3, m)
+    x0 = host.test_vector(seed, 4, n) if x_in is None else x_in
+    ref = oracle.aprod2(L, a, idx, y, x0.copy(), threads=threads)
+    xg = dev(x0)
+    gsr.gsr_aprod2(sys_, dev(y), xg)
+    got = xg.cpu().numpy()
+    assert np.linalg.norm(got - ref) <= 1e-11 * np.linalg.norm(ref)
+    inc = ref - x0
+    for name, sl in blocks_of(shape).items():
+        if sl.stop > sl.start and np.linalg.norm(inc[sl]) > 0:
+            e = np.linalg.norm(got[sl] - ref[sl])
+            assert e <= 1e-11 * np.linalg.norm(ref[sl]), f"aprod2 block {name}: {e / np.linalg.norm(ref[sl]):.3e}"
+    return got
+
+
+# ------------------------------------------------------------------ generator
+def test_device_generator_matches_host():
+    for shape in (C1, C3.scaled(3000), C5.scaled(60, n_knots=200, n_instr=40, n_constraint_rows=10)):
+        a, idx = host.make_rows(shape)
+        va, vi = gdev.make_system(shape)
+        assert tuple(va.shape) == a.shape and tuple(vi.shape) == idx.shape
+        assert np.array_equal(vi.cpu().numpy(), idx)                    # integer outputs: bit-identical
+        np.testing.assert_allclose(va.cpu().numpy(), a, rtol=1e-13, atol=1e-15)
+    np.testing.assert_allclose(gdev.x_true(C1).cpu().numpy(), host.x_true(C1), rtol=1e-13, atol=1e-15)
+    np.testing.assert_allclose(gdev.noise(C1, 20000).cpu().numpy(), host.noise(C1, 0, 20000), rtol=1e-13, atol=1e-21)
+
+
+# ------------------------------------------------------------------ aprod, C1 and edge cases
+def test_aprod_c1():
+    a, idx = host.make_rows(C1)
+    with make_gpu_system(C1, a, idx) as s:
+        assert s.n_rows == 20000 and s.n_unknowns == 8061
+        for seed in (1, 2, 3):
+            check_aprod1(C1, a, idx, s, seed)
+            check_aprod2(C1, a, idx, s, seed)
+        # zero initial output: pure products
+        check_aprod1(C1, a, idx, s, 5, y_in=np.zeros(20000))
+        check_aprod2(C1, a, idx, s, 5, x_in=np.zeros(8061))
+
+
+@pytest.mark.parametrize("n_stars,obs", [(1, 1), (1, 31), (1, 33), (3, 11), (7, 37), (5, 129), (2, 1000), (64, 64)])
+def test_aprod_ragged_sizes(n_stars, obs):
+    """Row counts around the 32-row tile: single row, ragged tails, several tiles, one long star."""
+    shape = tiny_shape(n_stars=n_stars, obs=obs, n_knots=50, n_instr=17, seed=100 + obs)
+    a, idx = host.make_rows(shape)
+    with make_gpu_system(shape, a, idx) as s:
+        check_aprod1(shape, a, idx, s)
+        check_aprod2(shape, a, idx, s)
+
+
+def test_aprod_skewed_stars_and_hot_knots():
+    shape = C3.scaled(4000)                       # power-law rows per star, hot attitude knots
+    a, idx = host.make_rows(shape)
+    assert np.bincount(idx[:, 0]).max() > 500
+    with make_gpu_system(shape, a, idx) as s:
+        check_aprod1(shape, a, idx, s)
+        check_aprod2(shape, a, idx, s)
+
+
+def test_aprod_constraint_rows():
+    shape = C5.scaled(300, n_knots=600, n_instr=40, n_constraint_rows=100)
+    a, idx = host.make_rows(shape)
+    with make_gpu_system(shape, a, idx) as s:
+        check_aprod1(shape, a, idx, s)
+        check_aprod2(shape, a, idx, s)
+
+
+def test_aprod_n_glob_zero_and_edges():
+    shape = tiny_shape(n_stars=9, obs=50, n_knots=12, n_instr=6, n_glob=0, seed=77)
+    a, idx = host.make_rows(shape)
+    idx[::3, 1] = shape.n_knots - 4                       # upper edge of att_start
+    idx[::5, 1] = 0
+    idx[1::7, 2:8] = np.array([2, 2, 5, 2, 0, 5], dtype=np.int32)   # repeated instrumental columns
+    with make_gpu_system(shape, a, idx) as s:
+        assert s.n_unknowns == 45 + 36 + 6
+        check_aprod1(shape, a, idx, s)
+        check_aprod2(shape, a, idx, s)
+    # a block of zero coefficients leaves its part of x bitwise untouched
+    a2 = a.copy()
+    a2[:, 5:17] = 0.0
+    with make_gpu_system(shape, a2, idx) as s:
+        x0 = host.test_vector(9, 1, shape.n_unknowns)
+        xg = dev(x0)
+        gsr.gsr_aprod2(s, dev(host.test_vector(9, 2, a.shape[0])), xg)
+        sl = blocks_of(shape)["att"]
+        assert np.array_equal(xg.cpu().numpy()[sl], x0[sl])
+
+
+def test_aprod_accumulates():
+    a, idx = host.make_rows(C1)
+    L = oracle.layout_of(C1)
+    x = host.test_vector(11, 1, C1.n_unknowns)
+    with make_gpu_system(C1, a, idx) as s:
+        y = torch.zeros(20000, dtype=torch.float64, device=DEV)
+        xd = dev(x)
+        s.aprod1(xd, y)
+        once = y.cpu().numpy().copy()
+        s.aprod1(xd, y)
+        twice = y.cpu().numpy()
+        bound = oracle.aprod1_abs(L, a, idx, x)
+        assert np.all(np.abs(twice - 2 * once) <= 4e-13 * bound)
+        assert np.array_equal(xd.cpu().numpy(), x)              # input untouched
+        # bit-reproducible run to run
+        y2 = torch.zeros(20000, dtype=torch.float64, device=DEV)
+        s.aprod1(xd, y2)
+        assert np.array_equal(y2.cpu().numpy(), once)
+
+
+def test_empty_system_and_errors():
+    shape = tiny_shape(n_stars=2, obs=3, n_knots=8, n_instr=6)
+    a, idx = host.make_rows(shape)
+    s0 = gsr.gsr_create(2, 8, 6, 1, torch.empty((0, 24), dtype=torch.float64, device=DEV),
+                        torch.empty((0, 8), dtype=torch.int32, device=DEV))
+    x = torch.ones(s0.n_unknowns, dtype=torch.float64, device=DEV)
+    s0.aprod2(torch.empty(0, dtype=torch.float64, device=DEV), x)
+    assert bool((x == 1).all())
+    s0.destroy()
+    for col, val in ((0, 5), (0, -1), (1, shape.n_knots - 3), (1, -1), (4, shape.n_instr), (7, -2)):
+        bad = idx.copy()
+        bad[2, col] = val
+        with pytest.raises(gsr.GsrError) as ei:
+            make_gpu_system(shape, a, bad)
+        assert ei.value.code == -2
+    bad = idx.copy()
+    bad[[1, 4], 0] = bad[[4, 1], 0]                         # stars out of order
+    with pytest.raises(gsr.GsrError) as ei:
+        make_gpu_system(shape, a, bad)
+    assert ei.value.code == -2
+    with pytest.raises(gsr.GsrError) as ei:                 # n_glob must be 0 or 1
+        gsr.gsr_create(2, 8, 6, 2, dev(a), dev(idx))
+    assert ei.value.code == -1
+    big = torch.zeros(a.size + 1, dtype=torch.float64, device=DEV)
+    mis = big[1:].view(-1, 24)                              # 8-byte aligned only
+    mis.copy_(dev(a))
+    with pytest.raises(gsr.GsrError) as ei:
+        gsr.gsr_create(2, 8, 6, 1, mis, dev(idx))
+    assert ei.value.code == -1
+    with pytest.raises(TypeError):                          # CPU tensors are refused: no CPU fallback
+        gsr.gsr_create(2, 8, 6, 1, torch.from_numpy(a), torch.from_numpy(idx))
+
+
+# ------------------------------------------------------------------ LSQR
+def gpu_state(s, m, n):
+    u = torch.empty(m, dtype=torch.float64, device=DEV)
+    v, w, x = (torch.empty(n, dtype=torch.float64, device=DEV) for _ in range(3))
+    sc = s.lsqr_state(u, v, w, x)
+    return {"u": u.cpu().numpy(), "v": v.cpu().numpy(), "w": w.cpu().numpy(), "x": x.cpu().numpy()}, sc
+
+
+def oracle_state_from(vecs, sc, m, n):
+    st = oracle.LsqrState(m, n)
+    for k in ("u", "v", "w", "x"):
+        getattr(st, k)[:] = vecs[k]
+    for k, val in sc.items():
+        setattr(st, k, val)
+    return st
+
+
+def replay_one_step(shape, a, idx, s, tol_vec=1e-11, tol_sc=1e-10, threads=1):
+    """GPU state at k -> one ORACLE iteration -> must equal the GPU state at k+1."""
+    L = oracle.layout_of(shape)
+    m, n = a.shape[0], shape.n_unknowns
+    vecs, sc = gpu_state(s, m, n)
+    st = oracle_state_from(vecs, sc, m, n)
+    oracle.lsqr_step(L, a, idx, st, threads=threads)
+    s.lsqr_iterate(1)
+    vecs1, sc1 = gpu_state(s, m, n)
+    assert sc1["itn"] == st.itn
+    for k in ("u", "v", "w", "x"):
+        ref = getattr(st, k)
+        e = np.linalg.norm(vecs1[k] - ref) / np.linalg.norm(ref)
+        assert e <= tol_vec, f"one-step replay at itn {st.itn}: vector {k} off by {e:.3e}"
+    for k in ("alpha", "beta", "rhobar", "phibar", "rnorm", "arnorm", "anorm", "acond", "ddnorm", "xnorm",
+              "xxnorm", "z", "cs2", "sn2", "bnorm"):
+        ref = getattr(st, k)
+        assert abs(sc1[k] - ref) <= tol_sc * abs(ref) + 1e-300, f"one-step replay at itn {st.itn}: {k} {sc1[k]} vs {ref}"
+
+
+def test_lsqr_c1_to_convergence():
+    a, idx = host.make_rows(C1)
+    L = oracle.layout_of(C1)
+    xt = host.x_true(C1)
+    b = rhs(C1, a, idx, xt)
+    xr, rr = oracle.lsqr(L, a, idx, b, itnlim=5000, atol=1e-12, btol=1e-12, conlim=1e8)
+    with make_gpu_system(C1, a, idx) as s:
+        x = torch.empty(C1.n_unknowns, dtype=torch.float64, device=DEV)
+        res = s.lsqr(dev(b), x, 5000, 1e-12, 1e-12, 1e8)
+        xg = x.cpu().numpy()
+        assert res.istop == rr["istop"] == 2
+        assert abs(res.itn - rr["itn"]) <= max(3, 0.02 * rr["itn"])
+        assert np.linalg.norm(xg - xr) <= 1e-9 * np.linalg.norm(xr)
+        # anorm / acond accumulate over iterations, so they depend on where each run stopped
+        for k, tol in (("r1norm", 1e-2), ("xnorm", 1e-6), ("anorm", 0.1), ("acond", 0.15)):
+            assert abs(getattr(res, k) - rr[k]) <= tol * rr[k]
+        assert abs(res.bnorm - rr["bnorm"]) <= 1e-13 * rr["bnorm"]
+        # the recurrence estimate matches the true residual of the GPU solution (oracle aprod1)
+        r = b - oracle.aprod1(L, a, idx, xg, np.zeros_like(b))
+        assert abs(np.linalg.norm(r) - res.r1norm) <= 1e-8 * np.linalg.norm(r)
+        ne = nonempty_columns(C1, idx)
+        assert np.all(xg[~ne] == 0.0)
+        assert np.linalg.norm(xg[ne] - xt[ne]) <= 1e-5 * np.linalg.norm(xt[ne])
+
+
+def test_lsqr_same_iteration_count_early_and_replays():
+    a, idx = host.make_rows(C1)
+    L = oracle.layout_of(C1)
+    b = rhs(C1, a, idx, host.x_true(C1))
+    with make_gpu_system(C1, a, idx) as s:
+        bd = dev(b)
+        x = torch.empty(C1.n_unknowns, dtype=torch.float64, device=DEV)
+        for k in (1, 2, 3, 4, 5):                       # literal "same iteration count" comparison
+            xr, rr = oracle.lsqr(L, a, idx, b, itnlim=k)
+            res = s.lsqr(bd, x, k)
+            assert res.istop == 7 and res.itn == k
+            assert np.linalg.norm(x.cpu().numpy() - xr) <= 1e-9 * np.linalg.norm(xr)
+            for name in ("r1norm", "anorm", "acond", "arnorm", "xnorm", "bnorm"):
+                assert abs(getattr(res, name) - rr[name]) <= 1e-9 * abs(rr[name])
+        # init state equals the oracle's
+        s.lsqr_init(bd)
+        vecs, sc = gpu_state(s, a.shape[0], C1.n_unknowns)
+        st0 = oracle.lsqr_init(L, a, idx, b)
+        for kk in ("u", "v", "w", "x"):
+            assert np.linalg.norm(vecs[kk] - getattr(st0, kk)) <= 1e-12 * max(np.linalg.norm(getattr(st0, kk)), 1e-300)
+        for kk in ("alpha", "beta", "rhobar", "phibar", "bnorm", "rnorm", "arnorm"):
+            assert abs(sc[kk] - getattr(st0, kk)) <= 1e-12 * abs(getattr(st0, kk))
+        # one-iteration replays along the trajectory (no chaotic amplification)
+        done = 0
+        for k in (0, 1, 7, 40, 150, 300):
+            s.lsqr_iterate(k - done)
+            replay_one_step(C1, a, idx, s)
+            done = k + 1
+
+
+def test_lsqr_stop_codes():
+    shape = tiny_shape(n_stars=20, obs=30, n_knots=12, n_instr=10, seed=5)
+    a, idx = host.make_rows(shape)
+    L = oracle.layout_of(shape)
+    n = shape.n_unknowns
+    with make_gpu_system(shape, a, idx) as s:
+        x = torch.full((n,), 7.0, dtype=torch.float64, device=DEV)
+        res = s.lsqr(torch.zeros(a.shape[0], dtype=torch.float64, device=DEV), x, 10)   # b = 0
+        assert res.istop == 0 and res.itn == 0 and not bool(x.any())
+        b = rhs(shape, a, idx, host.x_true(shape), noisy=False)                        # consistent system
+        xr, rr = oracle.lsqr(L, a, idx, b, itnlim=5000, atol=1e-14, btol=1e-14)
+        res = s.lsqr(dev(b), x, 5000, 1e-14, 1e-14, 0.0)
+        assert res.istop == rr["istop"] and res.istop in (1, 2)
+        assert np.linalg.norm(x.cpu().numpy() - xr) <= 1e-9 * np.linalg.norm(xr)
+        res = s.lsqr(dev(b), x, 3)
+        assert res.istop == 7 and res.itn == 3
+        res = s.lsqr(dev(b), x, 0)
+        assert res.istop == 7 and res.itn == 0 and not bool(x.any())
+        # the paper's "identity solution": b = A 1
+        b1 = rhs(shape, a, idx, np.ones(n), noisy=False)
+        xr, rr = oracle.lsqr(L, a, idx, b1, itnlim=5000, atol=1e-14, btol=1e-14)
+        res = s.lsqr(dev(b1), x, 5000, 1e-14, 1e-14, 0.0)
+        assert np.linalg.norm(x.cpu().numpy() - xr) <= 1e-9 * np.linalg.norm(xr)
+        # conlim exit (istop 3) fires on both sides at the same place
+        xr, rr = oracle.lsqr(L, a, idx, b, itnlim=5000, conlim=5.0)
+        res = s.lsqr(dev(b), x, 5000, 0.0, 0.0, 5.0)
+        assert res.istop == rr["istop"] == 3 and abs(res.itn - rr["itn"]) <= 1
+
+
+def test_lsqr_constraint_rows_to_convergence():
+    shape = C5.scaled(400, n_knots=300, n_instr=24, n_constraint_rows=60)
+    a, idx = host.make_rows(shape)
+    L = oracle.layout_of(shape)
+    b = rhs(shape, a, idx, host.x_true(shape))
+    xr, rr = oracle.lsqr(L, a, idx, b, itnlim=20000, atol=1e-12, btol=1e-12, conlim=1e8)
+    with make_gpu_system(shape, a, idx) as s:
+        x = torch.empty(shape.n_unknowns, dtype=torch.float64, device=DEV)
+        res = s.lsqr(dev(b), x, 20000, 1e-12, 1e-12, 1e8)
+        assert res.istop == rr["istop"]
+        assert np.linalg.norm(x.cpu().numpy() - xr) <= 1e-9 * np.linalg.norm(xr)
+
+
+def test_lsqr_host_entry_matches_device_entry():
+    a, idx = host.make_rows(C1)
+    b = rhs(C1, a, idx, host.x_true(C1))
+    xh = np.empty(C1.n_unknowns)
+    rh = gsr.gsr_lsqr_host(C1.n_stars, C1.n_knots, C1.n_instr, C1.n_glob, a, idx, b, xh, 50)
+    with make_gpu_system(C1, a, idx) as s:
+        x = torch.empty(C1.n_unknowns, dtype=torch.float64, device=DEV)
+        rd = s.lsqr(dev(b), x, 50)
+        n0 = s.launch_count()
+        assert n0 > 50 * 6
+    assert rh.istop == rd.istop == 7 and rh.itn == rd.itn == 50
+    assert np.linalg.norm(xh - x.cpu().numpy()) <= 1e-6 * np.linalg.norm(xh)   # (atomics reorder: R16)
+    assert abs(rh.bnorm - rd.bnorm) <= 1e-14 * rd.bnorm
+
+
+# ------------------------------------------------------------------ full-size C2 (the bench launch configuration)
+@pytest.fixture(scope="module")
+def c2_system():
+    vals, idx = gdev.make_system(C2)
+    s = gsr.gsr_create(C2.n_stars, C2.n_knots, C2.n_instr, C2.n_glob, vals, idx)
+    a_h, idx_h = vals.cpu().numpy(), idx.cpu().numpy()
+    yield s, vals, idx, a_h, idx_h
+    s.destroy()
+
+
+def test_c2_full_size_aprod(c2_system):
+    s, vals, idx, a, idx_h = c2_system
+    assert s.n_rows == 10_000_000 and s.n_unknowns == 560_601
+    th = oracle.max_threads()
+    check_aprod1(C2, a, idx_h, s, seed=21, threads=th)     # OpenMP oracle: same per-row arithmetic as serial
+    check_aprod2(C2, a, idx_h, s, seed=22, threads=th)
+    # sampled rows / columns against the serial oracle
+    L = oracle.layout_of(C2)
+    x = host.test_vector(23, 1, C2.n_unknowns)
+    yg = torch.zeros(s.n_rows, dtype=torch.float64, device=DEV)
+    s.aprod1(dev(x), yg)
+    for r0 in (0, 4_999_968, 9_999_000):
+        sl = slice(r0, r0 + 1000)
+        ref = oracle.aprod1(L, a[sl], idx_h[sl], x, np.zeros(1000))
+        bound = oracle.aprod1_abs(L, a[sl], idx_h[sl], x)
+        assert np.all(np.abs(yg[sl].cpu().numpy() - ref) <= 1e-13 * bound)
+
+
+def test_c2_lsqr_100_iterations(c2_system):
+    s, vals, idx, a, idx_h = c2_system
+    L = oracle.layout_of(C2)
+    th = oracle.max_threads()
+    xt = gdev.x_true(C2)
+    b = gdev.noise(C2, s.n_rows)
+    s.aprod1(xt, b)                                  # b = A x_true + noise (aprod1 parity checked above)
+    bh = b.cpu().numpy()
+    # literal same-iteration-count comparison while it is well-posed
+    x = torch.empty(s.n_unknowns, dtype=torch.float64, device=DEV)
+    xr, rr = oracle.lsqr(L, a, idx_h, bh, itnlim=3, threads=th)
+    res = s.lsqr(b, x, 3)
+    assert res.itn == 3 and np.linalg.norm(x.cpu().numpy() - xr) <= 1e-9 * np.linalg.norm(xr)
+    # 100 iterations as in configs[1]: replay iteration 100 -> 101 through the oracle
+    s.lsqr_init(b)
+    s.lsqr_iterate(100)
+    res = s.lsqr_result(x)
+    assert res.itn == 100 and res.istop == 0
+    xg = x.cpu().numpy()
+    r = bh - oracle.aprod1(L, a, idx_h, xg, np.zeros_like(bh), threads=th)
+    assert abs(np.linalg.norm(r) - res.r1norm) <= 1e-8 * np.linalg.norm(r)
+    replay_one_step(C2, a, idx_h, s, threads=th)
