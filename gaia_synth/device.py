@@ -50,8 +50,9 @@ def _stream():
     return torch.cuda.current_stream().cuda_stream
 
 
-def make_system(shape: C.SystemShape, device="cuda"):
-    """(values [M,24] float64, indices [M,8] int32) as CUDA tensors, generated in place in HBM."""
+def make_system(shape: C.SystemShape, device="cuda", r0: int = 0, r1: int = None):
+    """(values [M,24] float64, indices [M,8] int32) as CUDA tensors, generated in place in HBM.
+    r0/r1 select a row range (default: the whole system)."""
     import torch
     sptr_dev = None
     if shape.obs_per_star:
@@ -65,9 +66,11 @@ def make_system(shape: C.SystemShape, device="cuda"):
     if shape.hot_knots:
         ws, wlen = host.hot_windows(shape)
         hot_dev = torch.from_numpy(ws.astype(np.int64)).to(device)
-    vals = torch.empty((m, 24), dtype=torch.float64, device=device)
-    idx = torch.empty((m, 8), dtype=torch.int32, device=device)
-    rc = lib().gs_fill_rows(vals.data_ptr(), idx.data_ptr(), shape.seed, 0, m, m_obs, shape.n_constraint_rows,
+    r1 = m if r1 is None else min(r1, m)
+    nr = max(r1 - r0, 0)
+    vals = torch.empty((nr, 24), dtype=torch.float64, device=device)
+    idx = torch.empty((nr, 8), dtype=torch.int32, device=device)
+    rc = lib().gs_fill_rows(vals.data_ptr(), idx.data_ptr(), shape.seed, r0, nr, m_obs, shape.n_constraint_rows,
                             shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, shape.obs_per_star,
                             sptr_dev.data_ptr() if sptr_dev is not None else None, int(shape.hot_knots),
                             hot_dev.data_ptr() if hot_dev is not None else None, C.N_HOT_WINDOWS, wlen,
