@@ -28,6 +28,7 @@ struct EventPair {
 
 struct gsr_system {
   SysView v;
+  SideData side;
   Tuning tune;
   int device = 0;
   int num_sms = 148;
@@ -61,6 +62,32 @@ extern "C" const char* gsr_last_cuda_error(void) { return g_cuda_err; }
 extern "C" const char* gsr_version(void) { return "gsr-b200 0.1 (sm_100a)"; }
 
 static bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+    return cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
+  const cuuint64_t dims[2] = {(cuuint64_t)NSLOT, (cuuint64_t)(M > 0 ? M : 1)};
+  const cuuint64_t strides[1] = {(cuuint64_t)NSLOT * sizeof(double)};       // 192-byte rows
+  const cuuint32_t box[2] = {26u, 32u};                                      // 24 + 2 zero-filled pad columns
+  const cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(values),
+                                                   dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return GSR_ECUDA;
+  }
+  return GSR_OK;
+}
 
 extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* values,
                           const int32_t* indices, void* stream) {
@@ -97,6 +124,13 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
   cudaFree(flag);
   if (e != cudaSuccess) { delete s; return cuda_fail(e, "gsr_create validation"); }
   if (h != 0) { delete s; return GSR_ELAYOUT; }
+  // side structures: the row-tile tensor map and the expanded attitude-window table
+  if (v.M > 0) {
+    int rc = make_row_tensor_map(&s->side.map, values, v.M);
+    if (rc) { delete s; return rc; }
+  }
+  e = cudaMalloc(&s->side.xw, (size_t)(3 * (v.K - 3) * 4) * sizeof(double));
+  if (e != cudaSuccess) { delete s; cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc xw"); }
   *out = s;
   return GSR_OK;
 }
@@ -111,6 +145,7 @@ static void free_events(gsr_system* s) {
 extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
+  cudaFree(s->side.xw);
   free_events(s);
   delete s;
 }
@@ -143,7 +178,7 @@ static int do_aprod1(gsr_system* s, const double* x, double* y, const double* c0
                      int* done, cudaStream_t st) {
   EventPair ep;
   const bool p = prof_begin(s, 1, st, &ep);
-  cudaError_t e = launch_aprod1(s->v, s->tune, s->num_sms, x, y, c0, sumsq, done, st, &s->launches);
+  cudaError_t e = launch_aprod1(s->v, s->side, s->tune, s->num_sms, x, y, c0, sumsq, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod1 launch");
   return GSR_OK;
@@ -152,7 +187,7 @@ static int do_aprod2(gsr_system* s, const double* y, double* x, const double* ys
                      cudaStream_t st) {
   EventPair ep;
   const bool p = prof_begin(s, 2, st, &ep);
-  cudaError_t e = launch_aprod2(s->v, s->tune, s->num_sms, y, x, yscale, done, st, &s->launches);
+  cudaError_t e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, yscale, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod2 launch");
   return GSR_OK;
@@ -381,6 +416,8 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   if (!strcmp(name, "aprod1_variant")) s->tune.aprod1_variant = (int)value;
   else if (!strcmp(name, "aprod2_variant")) s->tune.aprod2_variant = (int)value;
   else if (!strcmp(name, "ctas_per_sm")) s->tune.ctas_per_sm = (int)value;
+  else if (!strcmp(name, "warps")) s->tune.warps = (int)value;
+  else if (!strcmp(name, "stages")) s->tune.stages = (int)value;
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;
   else return GSR_EINVAL;
   return GSR_OK;

@@ -1,5 +1,6 @@
 // Internal declarations of libgsr (not part of the ABI; the ABI is include/gsr.h).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -33,20 +34,30 @@ struct DevScalars {
 };
 
 struct Tuning {
-  int aprod1_variant = 0;
-  int aprod2_variant = 0;
-  int ctas_per_sm = 0;  // 0 = default of the variant
-  int check_every = 16; // LSQR iterations between host polls of the stop flag
+  int aprod1_variant = 1;  // 1 = TMA-staged tiles (default), 0 = one thread per row (simple)
+  int aprod2_variant = 1;  // 1 = TMA-staged tiles, split by parameter block (default), 0 = one thread per row
+  int ctas_per_sm = 0;     // 0 = default of the variant
+  int warps = 0;           // warps per CTA of the TMA kernels (0 = default 8)
+  int stages = 0;          // ring depth per warp (0 = default 3)
+  int check_every = 16;    // LSQR iterations between host polls of the stop flag
 };
+
+// Side structures owned by the library (built in gsr_create).
+struct SideData {
+  CUtensorMap map;         // 24 x M fp64 tensor, box 26 x 32 (tma.cuh)
+  double* xw = nullptr;    // expanded attitude windows, 3*(K-3)*4 doubles
+};
+
+constexpr size_t SMEM_BUDGET = 227 * 1024 - 512;   // dynamic shared memory we allow one CTA (static: block_sum)
 
 // Launchers (each returns cudaGetLastError()).  Null coefficient pointers mean 1.0 / "no".
 //   aprod1: y[r] = c1 * (A x)[r] + c0 * y[r]      (c0 = c1 = 1 -> Eq. 2);  *sumsq += sum y[r]^2
-cudaError_t launch_aprod1(const SysView& s, const Tuning& t, int num_sms, const double* x, double* y,
-                          const double* c0, double* sumsq, int* done, cudaStream_t st,
+cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* x,
+                          double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches);
 //   aprod2: x += A^T (yscale * y)
-cudaError_t launch_aprod2(const SysView& s, const Tuning& t, int num_sms, const double* y, double* x,
-                          const double* yscale, const int* done, cudaStream_t st, int64_t* launches);
+cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
+                          double* x, const double* yscale, const int* done, cudaStream_t st, int64_t* launches);
 cudaError_t launch_validate(const SysView& s, int* flag, cudaStream_t st, int64_t* launches);
 
 // LSQR vector / scalar kernels (lsqr_kernels.cu)

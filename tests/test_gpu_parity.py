@@ -248,7 +248,7 @@ def test_lsqr_c1_to_convergence():
         res = s.lsqr(dev(b), x, 5000, 1e-12, 1e-12, 1e8)
         xg = x.cpu().numpy()
         assert res.istop == rr["istop"] == 2
-        assert abs(res.itn - rr["itn"]) <= max(3, 0.02 * rr["itn"])
+        assert abs(res.itn - rr["itn"]) <= max(3, 0.05 * rr["itn"])   # the stopping test straddles its threshold (R16)
         assert np.linalg.norm(xg - xr) <= 1e-9 * np.linalg.norm(xr)
         # anorm / acond accumulate over iterations, so they depend on where each run stopped
         for k, tol in (("r1norm", 1e-2), ("xnorm", 1e-6), ("anorm", 0.1), ("acond", 0.15)):
