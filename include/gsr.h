@@ -143,10 +143,11 @@ int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int
 
 /* ---- diagnostics ----------------------------------------------------------------------------
  * gsr_launch_count : kernels launched by this system object so far (host out-pointer).
- * gsr_profile      : enable (1) / disable (0) CUDA-event timing of the aprod1 / aprod2 kernels
- *                    issued by gsr_lsqr_iterate and gsr_aprod1/2 on their own stream.
+ * gsr_profile      : enable (1) / disable (0) CUDA-event timing of the matrix-pass kernels issued by
+ *                    gsr_lsqr_iterate and gsr_aprod1/2, on their own stream.
  * gsr_profile_get  : after a synchronise, mean duration in ms and launch count since the last
- *                    call, per kernel class: which = 1 aprod1, 2 aprod2 (host out-pointers).
+ *                    call, per kernel class: which = 1 aprod1, 2 aprod2, 3 the fused LSQR pass
+ *                    (aprod 1 + aprod 2 of one iteration in one sweep over A) (host out-pointers).
  * gsr_set_option   : tuning knobs; unknown names -> GSR_EINVAL.          */
 int gsr_launch_count(const gsr_system *sys, int64_t *n_launches);
 int gsr_profile(gsr_system *sys, int enable);

@@ -1,28 +1,15 @@
-// aprod1:  y[r] = c1 * sum_k a[r][k] * x[col(r,k)] + c0 * y[r]      (Eq. 2)
+// aprod1:  y[r] = sum_k a[r][k] * x[col(r,k)] + c0 * y[r]           (Eq. 2)
 // with the LSQR u-update and ||u||^2 fused in.
-#include "gsr_internal.cuh"
-#include "tma.cuh"
+#include "aprod_device.cuh"
 
 namespace gsr {
 
 // ---- variant 1 (default): TMA-staged row tiles, one warp per tile, lane per row -----------------
-// Data movement per row: 192 B coefficients + 32 B index record arrive by TMA (tma.cuh); the lane
-// reads them conflict-free from shared memory.  Gathers from x:
-//   astro  : x[5*star .. +4]   (rows are sorted by star: the lanes of a warp share 1-2 stars)
-//   att    : ONE 32-byte load per axis from the expanded window table xw[ax][t] = x[t..t+3]
-//            (k_expand_att below; 12 scalar gathers per row would saturate the L1 tag pipe)
-//   instr  : shared-memory copy of the instrumental slice when it fits, else L2 gathers
-//   global : one register.
-// y[r] <- (A x)[r] + c0 * y[r], sum of squares accumulated for ||u|| (LSQR fusion).
-__device__ __forceinline__ void ld_nc_v4(const double* p, double& a, double& b, double& c, double& d) {
-  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
-}
-
-template <int STAGES, bool INSTR_SMEM>
+template <int ATT, bool GSMEM>
 __global__ void __launch_bounds__(512, 1)
-k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* __restrict__ x,
-             const double* __restrict__ xw, double* __restrict__ y, const double* __restrict__ c0p,
-             double* sumsq, int* done) {
+k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ x,
+             const double* __restrict__ xw, int64_t xw_axis_stride, double* __restrict__ y,
+             const double* __restrict__ c0p, double* sumsq, int* done) {
   if (done) {
     const int d = *done;
     if (d) {  // LSQR already stopped: no-op (and latch "update pending" 2 -> 1, see k_step_scalars)
@@ -31,23 +18,21 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* _
     }
   }
   extern __shared__ char smem_raw[];
-  char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  char* smem = smem_align128(smem_raw);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  char* ring_mem = smem + (size_t)warp * STAGES * STAGE_BYTES;
-  double* xi_s = reinterpret_cast<double*>(smem + (size_t)nwarps * STAGES * STAGE_BYTES);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<char*>(xi_s) + (INSTR_SMEM ? ((s.I * 8 + 15) & ~15ll) : 0));
+  char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
+  double* xi_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
 
-  TileRing<STAGES> ring;
+  TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
-  ring.init(ring_mem, bars + warp * STAGES, &map, s.idx, s.M, gw, W, lane);
-  if (INSTR_SMEM) {
+  ring.init(ring_mem, bars + warp * nstages, &map, s.idx, s.M, gw, W, lane, nstages);
+  if (GSMEM) {
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(x + s.oI + i);
     __syncthreads();
   }
+  GatherCtx gc{x, xw, xw_axis_stride, xi_s, x + s.oI, s.G ? __ldg(x + s.oG) : 0.0};
   const double c0 = c0p ? *c0p : 1.0;
-  const double xg = s.G ? __ldg(x + s.oG) : 0.0;
-  const int64_t Kw = s.K - 3;           // windows per axis in xw
-  const double* xi_g = x + s.oI;
   double sq = 0.0;
 
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
@@ -55,43 +40,7 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* _
     const bool valid = r < s.M;
     const double yin = valid ? y[r] : 0.0;
     const char* tile = ring.acquire();
-    const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
-    const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
-    int4 i0 = ip[0], i1 = ip[1];
-    if (!valid) { i0 = make_int4(0, 0, 0, 0); i1 = i0; }   // tail lanes: coefficients are zero-filled
-    double a[NSLOT];
-#pragma unroll
-    for (int q = 0; q < NSLOT / 2; q++) {
-      const double2 v = ap[q];
-      a[2 * q] = v.x;
-      a[2 * q + 1] = v.y;
-    }
-    // gathers
-    const double* xa = x + 5 * (int64_t)i0.x;
-    double g[NSLOT - 1];
-#pragma unroll
-    for (int k = 0; k < 5; k++) g[k] = __ldg(xa + k);
-    const double* w0 = xw + (int64_t)i0.y * 4;
-    ld_nc_v4(w0, g[5], g[6], g[7], g[8]);
-    ld_nc_v4(w0 + Kw * 4, g[9], g[10], g[11], g[12]);
-    ld_nc_v4(w0 + Kw * 8, g[13], g[14], g[15], g[16]);
-    if (INSTR_SMEM) {
-      g[17] = xi_s[i0.z]; g[18] = xi_s[i0.w]; g[19] = xi_s[i1.x];
-      g[20] = xi_s[i1.y]; g[21] = xi_s[i1.z]; g[22] = xi_s[i1.w];
-    } else {
-      g[17] = __ldg(xi_g + i0.z); g[18] = __ldg(xi_g + i0.w); g[19] = __ldg(xi_g + i1.x);
-      g[20] = __ldg(xi_g + i1.y); g[21] = __ldg(xi_g + i1.z); g[22] = __ldg(xi_g + i1.w);
-    }
-    double acc0 = a[23] * xg, acc1 = 0.0, acc2 = 0.0;
-#pragma unroll
-    for (int k = 0; k < 21; k += 3) {
-      acc0 = fma(a[k], g[k], acc0);
-      acc1 = fma(a[k + 1], g[k + 1], acc1);
-      acc2 = fma(a[k + 2], g[k + 2], acc2);
-    }
-    acc0 = fma(a[21], g[21], acc0);
-    acc1 = fma(a[22], g[22], acc1);
-    const double out = fma(c0, yin, (acc0 + acc1) + acc2);
+    const double out = fma(c0, yin, tile_row_dot<ATT, GSMEM>(tile, lane, valid, gc));
     if (valid) {
       y[r] = out;
       sq = fma(out, out, sq);
@@ -104,29 +53,72 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* _
   }
 }
 
-// xw[(ax*(K-3) + t)*4 + j] = x[oA + ax*K + t + j]   (t = 0 .. K-4): every possible 4-knot run as one
-// aligned 32-byte record, rebuilt from x at every aprod1 call (3K reads, 12K writes: << the matrix).
-__global__ void __launch_bounds__(256) k_expand_att(const double* __restrict__ xatt, int64_t K, double* __restrict__ xw,
-                                                    const int* done) {
+// Expanded attitude windows, rebuilt from x before every gather pass (3K reads, <= 12K writes: << matrix).
+//   step 1 (ATT_FULL): xw[(ax*nwin + t)*4 + j] = x[oA + ax*K + t + j],  t = 0 .. K-4
+//   step 2 (ATT_HALF): xw[(ax*nwin + w)*4 + j] = x[oA + ax*K + 2w + j], w = 0 .. (K-2)/2
+// Elements past the end of x (only pad slots of the very last windows) read as 0.
+__global__ void __launch_bounds__(256) k_expand_att(const double* __restrict__ x, int64_t oA, int64_t n, int64_t K,
+                                                    int step, int64_t nwin, double* __restrict__ xw, const int* done) {
   if (done && *done) return;
-  const int64_t Kw = K - 3, total = 3 * Kw;
+  const int64_t total = 3 * nwin;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t ax = i / Kw, t = i - ax * Kw;
-    const double* p = xatt + ax * K + t;
+    const int64_t ax = i / nwin, w = i - ax * nwin;
+    const int64_t e = oA + ax * K + w * step;
+    double v[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++) v[j] = (e + j < n) ? __ldg(x + e + j) : 0.0;
     double2* o = reinterpret_cast<double2*>(xw + i * 4);
-    o[0] = make_double2(__ldg(p), __ldg(p + 1));
-    o[1] = make_double2(__ldg(p + 2), __ldg(p + 3));
+    o[0] = make_double2(v[0], v[1]);
+    o[1] = make_double2(v[2], v[3]);
   }
 }
 
-// ---- variant 0: one thread per row, direct global loads (first correct path) -----------------
+cudaError_t launch_expand_att(const SysView& s, const SideData& sd, int num_sms, const double* x, const int* done,
+                              cudaStream_t st, int64_t* launches) {
+  const int64_t total = 3 * sd.xw_nwin;
+  int64_t eb = (total + 255) / 256;
+  if (eb > num_sms * 8) eb = num_sms * 8;
+  k_expand_att<<<(unsigned)eb, 256, 0, st>>>(x, s.oA, s.n, s.K, sd.att_mode == ATT_FULL ? 1 : 2, sd.xw_nwin, sd.xw, done);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// ---- shared-memory plan of the TMA kernels --------------------------------------------------------
+static size_t ring_bytes(int w, int st) { return (size_t)w * st * STAGE_BYTES + (size_t)(w * st + 2) * 8 + 128; }
+
+SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
+  SmemPlan p;
+  p.warps = t.warps > 0 ? t.warps : 8;
+  p.stages = t.stages > 0 ? t.stages : 2;
+  p.gather_smem = p.acc_smem = false;
+  const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
+  size_t ring = ring_bytes(p.warps, p.stages);
+  size_t left = SMEM_BUDGET > ring ? SMEM_BUDGET - ring : 0;
+  // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1 gathers per row
+  if ((what & PLAN_APROD2) && table <= left) { p.acc_smem = true; left -= table; }
+  if ((what & PLAN_APROD1) && table <= left) { p.gather_smem = true; left -= table; }
+  p.bytes = SMEM_BUDGET - left;
+  return p;
+}
+
+template <int ATT>
+static cudaError_t launch_tma1(bool gsmem, const SysView& s, const SideData& sd, int grid, const SmemPlan& p,
+                               const double* x, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st) {
+  auto k = gsmem ? k_aprod1_tma<ATT, true> : k_aprod1_tma<ATT, false>;
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+  if (e != cudaSuccess) return e;
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, x, sd.xw, sd.xw_axis_stride, y, c0, sumsq, done);
+  return cudaGetLastError();
+}
+
+// ---- variant 0: one thread per row, direct global loads (simple device-side cross-check) --------
 __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const double* __restrict__ x,
                                                           double* __restrict__ y,
                                                           const double* __restrict__ c0p,
                                                           double* sumsq, int* done) {
   if (done) {
     const int d = *done;
-    if (d) {  // LSQR already stopped: no-op (and latch "update pending" 2 -> 1, see k_step_scalars)
+    if (d) {
       if (d == 2 && blockIdx.x == 0 && threadIdx.x == 0) *done = 1;
       return;
     }
@@ -172,47 +164,19 @@ __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const doubl
   }
 }
 
-template <int STAGES, bool INSTR_SMEM>
-static cudaError_t launch_tma1(const SysView& s, const SideData& sd, int grid, int warps, size_t smem,
-                               const double* x, double* y, const double* c0, double* sumsq, int* done,
-                               cudaStream_t st) {
-  auto k = k_aprod1_tma<STAGES, INSTR_SMEM>;
-  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  k<<<grid, warps * 32, smem, st>>>(sd.map, s, x, sd.xw, y, c0, sumsq, done);
-  return cudaGetLastError();
-}
-
 cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* x,
                           double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
   if (t.aprod1_variant == 1) {
-    // expanded attitude windows, then the streaming kernel
-    const int64_t total = 3 * (s.K - 3);
-    int64_t eb = (total + 255) / 256;
-    if (eb > num_sms * 8) eb = num_sms * 8;
-    k_expand_att<<<(unsigned)eb, 256, 0, st>>>(x + s.oA, s.K, sd.xw, done);
-    ++*launches;
-    cudaError_t e = cudaGetLastError();
+    const SmemPlan p = plan_smem(s, t, PLAN_APROD1);
+    if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
+    cudaError_t e = launch_expand_att(s, sd, num_sms, x, done, st, launches);
     if (e != cudaSuccess) return e;
-    const int warps = t.warps > 0 ? t.warps : 8;
-    const int stages = t.stages > 0 ? t.stages : 3;
-    const size_t ring = (size_t)warps * stages * STAGE_BYTES + (size_t)warps * stages * 8 + 128 + 16;
-    if (ring > SMEM_BUDGET || warps > 16) return cudaErrorInvalidValue;
-    const size_t instr = (size_t)((s.I * 8 + 15) & ~15ll);
-    const bool ismem = ring + instr <= SMEM_BUDGET;
-    const size_t smem = ring + (ismem ? instr : 0);
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
     ++*launches;
-#define GSR_A1(ST) (ismem ? launch_tma1<ST, true>(s, sd, grid, warps, smem, x, y, c0, sumsq, done, st) \
-                          : launch_tma1<ST, false>(s, sd, grid, warps, smem, x, y, c0, sumsq, done, st))
-    switch (stages) {
-      case 2: return GSR_A1(2);
-      case 4: return GSR_A1(4);
-      default: return GSR_A1(3);
-    }
-#undef GSR_A1
+    return sd.att_mode == ATT_FULL ? launch_tma1<ATT_FULL>(p.gather_smem, s, sd, grid, p, x, y, c0, sumsq, done, st)
+                                   : launch_tma1<ATT_HALF>(p.gather_smem, s, sd, grid, p, x, y, c0, sumsq, done, st);
   }
   const int threads = 256;
   int64_t blocks = (s.M + threads - 1) / threads;

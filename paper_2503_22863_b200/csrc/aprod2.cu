@@ -1,40 +1,32 @@
 // aprod2:  x[col(r,k)] += a[r][k] * (yscale * y[r])                  (Eq. 3)
-#include "gsr_internal.cuh"
-#include "tma.cuh"
+#include "aprod_device.cuh"
 
 namespace gsr {
 
-// ---- variant 1 (default): TMA-staged row tiles, split by parameter block ------------------------
-//  astro  (slots 0-4)  : rows are sorted by star, so the lanes of a warp hold runs of equal star;
-//                        a segmented warp scan (shuffles) sums each run, the run head issues 5 adds.
-//  att    (slots 5-16) : the 12 x 32 products of a tile are walked element-per-lane, so 4 consecutive
-//                        lanes cover one 4-knot run: the 4 fp64 reductions of a run travel to L2 as
-//                        one request (measured 2.2x the add rate of lane-per-row issue).
-//  instr  (slots 17-22): block-privatised accumulators in shared memory (when the slice fits),
-//                        flushed to x once per CTA at the end; else reductions at L2.
-//  global (slot 23)    : register accumulation, one reduction per CTA.
-template <int STAGES, bool INSTR_SMEM>
+// ---- variant 1 (default): TMA-staged row tiles, split by parameter block (tile_scatter) ---------
+template <bool ASMEM>
 __global__ void __launch_bounds__(512, 1)
-k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* __restrict__ y,
-             double* __restrict__ x, const double* __restrict__ yscale, const int* done) {
+k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
+             double* __restrict__ x, double* ins_copies, int n_copies, const double* __restrict__ yscale,
+             const int* done) {
   if (done && *done) return;
   extern __shared__ char smem_raw[];
-  char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  char* smem = smem_align128(smem_raw);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  char* ring_mem = smem + (size_t)warp * STAGES * STAGE_BYTES;
-  double* acc_s = reinterpret_cast<double*>(smem + (size_t)nwarps * STAGES * STAGE_BYTES);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<char*>(acc_s) + (INSTR_SMEM ? ((s.I * 8 + 15) & ~15ll) : 0));
+  char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
+  double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
 
-  TileRing<STAGES> ring;
+  TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
-  ring.init(ring_mem, bars + warp * STAGES, &map, s.idx, s.M, gw, W, lane);
-  if (INSTR_SMEM) {
+  ring.init(ring_mem, bars + warp * nstages, &map, s.idx, s.M, gw, W, lane, nstages);
+  if (ASMEM) {
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
     __syncthreads();
   }
+  ScatterCtx sc{x, x + s.oA, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : x + s.oI,
+                acc_s, s.K};
   const double ys = yscale ? *yscale : 1.0;
-  double* xatt = x + s.oA;
-  double* xins = x + s.oI;
   double gacc = 0.0;
 
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
@@ -44,59 +36,12 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* _
     const double yv = valid ? ys * y[r] : 0.0;
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     const char* tile = ring.acquire();
-    const double* td = reinterpret_cast<const double*>(tile);
-    const int32_t* ti = reinterpret_cast<const int32_t*>(tile + COEF_TILE_BYTES);
-
-    // ---- attitude: element e = 12*row + slot, 4 consecutive lanes = one run of 4 knots
-#pragma unroll
-    for (int it = 0; it < 12; it++) {
-      const int e = it * 32 + lane;
-      const int row = e / 12, sl = e - row * 12;
-      const double yy = __shfl_sync(0xffffffffu, yv, row);
-      if (row < nvalid) {
-        const double a = td[row * ROW_STRIDE_D + 5 + sl];
-        const int att = ti[row * 8 + 1];
-        atomicAdd(xatt + (int64_t)(sl >> 2) * s.K + att + (sl & 3), a * yy);
-      }
-    }
-
-    // ---- lane-per-row part: astro, instrumental, global
-    const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
-    const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
-    int4 i0 = ip[0], i1 = ip[1];
-    const double2 a01 = ap[0], a23 = ap[1], a45 = ap[2];
-    const double2 a1617 = ap[8], a1819 = ap[9], a2021 = ap[10], a2223 = ap[11];
-    int star = valid ? i0.x : (-1 - lane);
-    double p0 = a01.x * yv, p1 = a01.y * yv, p2 = a23.x * yv, p3 = a23.y * yv, p4 = a45.x * yv;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-      const int so = __shfl_down_sync(0xffffffffu, star, off);
-      const double q0 = __shfl_down_sync(0xffffffffu, p0, off), q1 = __shfl_down_sync(0xffffffffu, p1, off),
-                   q2 = __shfl_down_sync(0xffffffffu, p2, off), q3 = __shfl_down_sync(0xffffffffu, p3, off),
-                   q4 = __shfl_down_sync(0xffffffffu, p4, off);
-      if (lane + off < 32 && so == star) { p0 += q0; p1 += q1; p2 += q2; p3 += q3; p4 += q4; }
-    }
-    const int sprev = __shfl_up_sync(0xffffffffu, star, 1);
-    if (valid && (lane == 0 || sprev != star)) {   // head of a run of equal star
-      double* xa = x + 5 * (int64_t)star;
-      atomicAdd(xa, p0); atomicAdd(xa + 1, p1); atomicAdd(xa + 2, p2); atomicAdd(xa + 3, p3); atomicAdd(xa + 4, p4);
-    }
-    if (valid) {
-      const double v17 = a1617.y * yv, v18 = a1819.x * yv, v19 = a1819.y * yv, v20 = a2021.x * yv,
-                   v21 = a2021.y * yv, v22 = a2223.x * yv;
-      if (INSTR_SMEM) {
-        atomicAdd(acc_s + i0.z, v17); atomicAdd(acc_s + i0.w, v18); atomicAdd(acc_s + i1.x, v19);
-        atomicAdd(acc_s + i1.y, v20); atomicAdd(acc_s + i1.z, v21); atomicAdd(acc_s + i1.w, v22);
-      } else {
-        atomicAdd(xins + i0.z, v17); atomicAdd(xins + i0.w, v18); atomicAdd(xins + i1.x, v19);
-        atomicAdd(xins + i1.y, v20); atomicAdd(xins + i1.z, v21); atomicAdd(xins + i1.w, v22);
-      }
-      gacc = fma(a2223.y, yv, gacc);
-    }
+    gacc += tile_scatter<ASMEM>(tile, lane, valid, nvalid, yv, sc);
     ring.release(lane);
   }
-  if (INSTR_SMEM) {
+  if (ASMEM) {
     __syncthreads();
+    double* xins = x + s.oI;
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) {
       const double v = acc_s[i];
       if (v != 0.0) atomicAdd(xins + i, v);
@@ -108,7 +53,32 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, const double* _
   }
 }
 
-// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (first correct path) --
+// x_instr[i] += sum_c copies[c][i]; copies are cleared for the next call.
+// (The instrumental accumulator is replicated when it does not fit shared memory: 60,000 addresses
+//  hit by 3e9 reductions are contention-bound at L2 -- 159 vs 193 Gadd/s measured with >= 6e5 addresses.)
+__global__ void __launch_bounds__(256) k_fold_instr(double* __restrict__ xins, double* __restrict__ copies, int n_copies,
+                                                    int64_t I, const int* done) {
+  if (done && *done) return;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < I; i += (int64_t)gridDim.x * blockDim.x) {
+    double sum = 0.0;
+    for (int c = 0; c < n_copies; c++) {
+      sum += copies[(size_t)c * I + i];
+      copies[(size_t)c * I + i] = 0.0;
+    }
+    xins[i] += sum;
+  }
+}
+
+cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, const int* done, cudaStream_t st,
+                              int64_t* launches) {
+  int64_t b = (s.I + 255) / 256;
+  if (b > 148 * 4) b = 148 * 4;
+  k_fold_instr<<<(unsigned)b, 256, 0, st>>>(x + s.oI, sd.ins_copies, sd.n_copies, s.I, done);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check) ----
 __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const double* __restrict__ y,
                                                           double* __restrict__ x,
                                                           const double* __restrict__ yscale,
@@ -154,42 +124,24 @@ __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const doubl
   }
 }
 
-template <int STAGES, bool INSTR_SMEM>
-static cudaError_t launch_tma2_t(const SysView& s, const SideData& sd, int grid, int warps, size_t smem,
-                                 const double* y, double* x, const double* yscale, const int* done, cudaStream_t st) {
-  auto k = k_aprod2_tma<STAGES, INSTR_SMEM>;
-  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  k<<<grid, warps * 32, smem, st>>>(sd.map, s, y, x, yscale, done);
-  return cudaGetLastError();
-}
-static cudaError_t launch_tma2(int stages, bool ismem, const SysView& s, const SideData& sd, int grid, int warps,
-                               size_t smem, const double* y, double* x, const double* yscale, const int* done,
-                               cudaStream_t st) {
-#define GSR_A2(ST) (ismem ? launch_tma2_t<ST, true>(s, sd, grid, warps, smem, y, x, yscale, done, st) \
-                          : launch_tma2_t<ST, false>(s, sd, grid, warps, smem, y, x, yscale, done, st))
-  switch (stages) {
-    case 2: return GSR_A2(2);
-    case 4: return GSR_A2(4);
-    default: return GSR_A2(3);
-  }
-#undef GSR_A2
-}
-
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
                           double* x, const double* yscale, const int* done, cudaStream_t st, int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
   if (t.aprod2_variant == 1) {
-    const int warps = t.warps > 0 ? t.warps : 8;
-    const int stages = t.stages > 0 ? t.stages : 3;
-    const size_t ring = (size_t)warps * stages * STAGE_BYTES + (size_t)warps * stages * 8 + 128 + 16;
-    if (ring > SMEM_BUDGET || warps > 16) return cudaErrorInvalidValue;
-    const size_t instr = (size_t)((s.I * 8 + 15) & ~15ll);
-    const bool ismem = ring + instr <= SMEM_BUDGET;
-    const size_t smem = ring + (ismem ? instr : 0);
+    const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
+    if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
+    auto k = p.acc_smem ? k_aprod2_tma<true> : k_aprod2_tma<false>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+    if (e != cudaSuccess) return e;
+    const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
+    k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, use_copies ? sd.ins_copies : nullptr, sd.n_copies,
+                                            yscale, done);
     ++*launches;
-    return launch_tma2(stages, ismem, s, sd, grid, warps, smem, y, x, yscale, done, st);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (use_copies) return launch_fold_instr(s, sd, x, done, st, launches);
+    return cudaSuccess;
   }
   const int threads = 256;
   int64_t blocks = (s.M + threads - 1) / threads;

@@ -34,15 +34,15 @@ struct gsr_system {
   int num_sms = 148;
   int64_t launches = 0;
   // LSQR workspace (allocated on first use)
-  double *u = nullptr, *vv = nullptr, *w = nullptr, *x = nullptr;
+  double *u = nullptr, *vv = nullptr, *w = nullptr, *x = nullptr, *g = nullptr;
   DevScalars* sc = nullptr;
   bool lsqr_ready = false;   // gsr_lsqr_init has run
   // profiling
   bool profile = false;
   std::vector<EventPair> pending;
   std::vector<EventPair> pool;
-  double prof_ms[3] = {0, 0, 0};
-  int64_t prof_n[3] = {0, 0, 0};
+  double prof_ms[4] = {0, 0, 0, 0};
+  int64_t prof_n[4] = {0, 0, 0, 0};
 };
 
 static inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
@@ -89,6 +89,35 @@ static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M
   return GSR_OK;
 }
 
+// (Re)allocate the expanded attitude-window table for the requested mode (0 = choose by size).
+static int build_att_table(gsr_system* s, int mode) {
+  const SysView& v = s->v;
+  const size_t full_bytes = (size_t)(3 * (v.K - 3)) * 32;
+  if (mode == 0) mode = full_bytes <= ATT_FULL_MAX_BYTES ? 1 : 2;
+  const int64_t nwin = mode == 1 ? v.K - 3 : (v.K - 2) / 2 + 1;
+  cudaFree(s->side.xw);
+  s->side.xw = nullptr;
+  cudaError_t e = cudaMalloc(&s->side.xw, (size_t)(3 * nwin * 4) * sizeof(double));
+  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc xw"); }
+  s->side.att_mode = mode;
+  s->side.xw_nwin = nwin;
+  s->side.xw_axis_stride = 4 * nwin;
+  return GSR_OK;
+}
+
+// Replicated instrumental accumulators, only when the slice cannot be privatised in shared memory.
+static int build_instr_copies(gsr_system* s) {
+  const SysView& v = s->v;
+  if ((size_t)v.I * 8 <= 96 * 1024) return GSR_OK;
+  const int copies = 8;
+  cudaError_t e = cudaMalloc(&s->side.ins_copies, (size_t)copies * v.I * sizeof(double));
+  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc ins_copies"); }
+  e = cudaMemset(s->side.ins_copies, 0, (size_t)copies * v.I * sizeof(double));
+  if (e != cudaSuccess) return cuda_fail(e, "cudaMemset ins_copies");
+  s->side.n_copies = copies;
+  return GSR_OK;
+}
+
 extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* values,
                           const int32_t* indices, void* stream) {
   if (!out) return GSR_EINVAL;
@@ -129,8 +158,9 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
     int rc = make_row_tensor_map(&s->side.map, values, v.M);
     if (rc) { delete s; return rc; }
   }
-  e = cudaMalloc(&s->side.xw, (size_t)(3 * (v.K - 3) * 4) * sizeof(double));
-  if (e != cudaSuccess) { delete s; cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc xw"); }
+  int rc2 = build_att_table(s, 0);
+  if (rc2 == GSR_OK) rc2 = build_instr_copies(s);
+  if (rc2) { gsr_destroy(s); return rc2; }
   *out = s;
   return GSR_OK;
 }
@@ -145,7 +175,7 @@ static void free_events(gsr_system* s) {
 extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
-  cudaFree(s->side.xw);
+  cudaFree(s->side.xw); cudaFree(s->side.ins_copies); cudaFree(s->g);
   free_events(s);
   delete s;
 }
@@ -211,9 +241,10 @@ static int ensure_workspace(gsr_system* s) {
       (e = cudaMalloc(&s->vv, n * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&s->w, n * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&s->x, n * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->g, n * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&s->sc, sizeof(DevScalars))) != cudaSuccess) {
-    cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
-    s->u = s->vv = s->w = s->x = nullptr; s->sc = nullptr;
+    cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->g); cudaFree(s->sc);
+    s->u = s->vv = s->w = s->x = s->g = nullptr; s->sc = nullptr;
     cudaGetLastError();
     return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc workspace");
   }
@@ -246,7 +277,22 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
   cudaStream_t st = S(stream);
   const int64_t n = s->v.n;
   DevScalars* sc = s->sc;
-  for (int64_t it = 0; it < n_iters; ++it) {
+  for (int64_t it = 0; it < n_iters && s->tune.fused; ++it) {
+    // 1+2 in one pass over A: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2 ; g = A^T u_hat
+    CU(cudaMemsetAsync(s->g, 0, (size_t)n * sizeof(double), st));
+    EventPair ep;
+    const bool p = prof_begin(s, 3, st, &ep);
+    cudaError_t e = launch_lsqr_fused(s->v, s->side, s->tune, s->num_sms, s->vv, s->u, s->g, &sc->c0_u, &sc->usq,
+                                      &sc->done, st, &s->launches);
+    if (p) prof_end(s, st, &ep);
+    if (e != cudaSuccess) return cuda_fail(e, "fused LSQR pass launch");
+    // beta ; v <- g / beta - beta v ; vsq = ||v||^2
+    CU(lsqr_launch_vcombine(s->vv, s->g, n, sc, st, &s->launches));
+    // 3-8: scalars, stopping rule ; then the x / w / v update
+    CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
+    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, st, &s->launches));
+  }
+  for (int64_t it = 0; it < n_iters && !s->tune.fused; ++it) {
     // 1: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2              (aprod 1)
     int rc = do_aprod1(s, s->vv, s->u, &sc->c0_u, &sc->usq, &sc->done, st);
     if (rc) return rc;
@@ -393,7 +439,7 @@ extern "C" int gsr_profile(gsr_system* s, int enable) {
 }
 
 extern "C" int gsr_profile_get(gsr_system* s, int which, double* mean_ms, int64_t* count) {
-  if (!s || which < 1 || which > 2) return GSR_EINVAL;
+  if (!s || which < 1 || which > 3) return GSR_EINVAL;
   for (auto& p : s->pending) {
     float ms = 0.f;
     cudaError_t e = cudaEventSynchronize(p.b);
@@ -418,6 +464,13 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "ctas_per_sm")) s->tune.ctas_per_sm = (int)value;
   else if (!strcmp(name, "warps")) s->tune.warps = (int)value;
   else if (!strcmp(name, "stages")) s->tune.stages = (int)value;
+  else if (!strcmp(name, "instr_copies")) s->tune.instr_copies = (int)value;
+  else if (!strcmp(name, "fused")) s->tune.fused = (int)value;
+  else if (!strcmp(name, "att_mode")) {
+    if (value < 0 || value > 2) return GSR_EINVAL;
+    cudaDeviceSynchronize();
+    return build_att_table(s, (int)value);
+  }
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;
   else return GSR_EINVAL;
   return GSR_OK;

@@ -1,0 +1,118 @@
+// One LSQR bidiagonalisation step in ONE pass over the matrix.
+//
+// Paige-Saunders (refs [29,30]):  beta u' = A v - alpha u ;  alpha' v' = A^T u' - beta v.
+// Row r's contribution to A^T u' needs only u'[r], which depends only on row r:
+//     uh[r] <- a_r . v + c0 * uh[r]          (uh = un-normalised u; c0 = -alpha/beta_prev)   "aprod 1"
+//     g     += a_r^T * uh[r]                 (g zeroed before the pass)                       "aprod 2"
+//     usq   += uh[r]^2
+// and afterwards, with beta = sqrt(usq):  v' (un-normalised) = g / beta - beta v   (n-length kernel).
+// Same arithmetic as running aprod1 then aprod2, but the 224 bytes of row r are streamed from HBM
+// once per iteration instead of twice, and staged / read from shared memory once.
+#include "aprod_device.cuh"
+
+namespace gsr {
+
+template <int ATT, bool GSMEM, bool ASMEM>
+__global__ void __launch_bounds__(512, 1)
+k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
+             const double* __restrict__ xw, int64_t xw_axis_stride, double* __restrict__ uh, double* __restrict__ g,
+             double* ins_copies, int n_copies, const double* __restrict__ c0p, double* usq, int* done) {
+  {
+    const int d = *done;
+    if (d) {  // LSQR already stopped: no-op (and latch "update pending" 2 -> 1, see k_step_scalars)
+      if (d == 2 && blockIdx.x == 0 && threadIdx.x == 0) *done = 1;
+      return;
+    }
+  }
+  extern __shared__ char smem_raw[];
+  char* smem = smem_align128(smem_raw);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
+  double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
+  double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : 0);
+
+  TileRing ring;
+  const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
+  ring.init(ring_mem, bars + warp * nstages, &map, s.idx, s.M, gw, W, lane, nstages);
+  if (ASMEM)
+    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
+  if (GSMEM)
+    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(v + s.oI + i);
+  if (ASMEM || GSMEM) __syncthreads();
+  GatherCtx gc{v, xw, xw_axis_stride, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
+  ScatterCtx sc{g, g + s.oA, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : g + s.oI,
+                acc_s, s.K};
+  const double c0 = *c0p;
+  double sq = 0.0, gacc = 0.0;
+
+  for (int64_t t = gw; t < ring.n_tiles; t += W) {
+    const int64_t row0 = t * TILE_ROWS;
+    const int64_t r = row0 + lane;
+    const bool valid = r < s.M;
+    const double uin = valid ? uh[r] : 0.0;
+    const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
+    const char* tile = ring.acquire();
+    double out = fma(c0, uin, tile_row_dot<ATT, GSMEM>(tile, lane, valid, gc));
+    if (valid) {
+      uh[r] = out;
+      sq = fma(out, out, sq);
+    } else {
+      out = 0.0;
+    }
+    gacc += tile_scatter<ASMEM>(tile, lane, valid, nvalid, out, sc);
+    ring.release(lane);
+  }
+  if (ASMEM) {
+    __syncthreads();
+    double* gins = g + s.oI;
+    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) {
+      const double a = acc_s[i];
+      if (a != 0.0) atomicAdd(gins + i, a);
+    }
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(usq, sq);
+  if (s.G) {
+    __syncthreads();
+    gacc = block_sum(gacc);
+    if (threadIdx.x == 0) atomicAdd(g + s.oG, gacc);
+  }
+}
+
+template <int ATT>
+static cudaError_t launch_fused_t(const SmemPlan& p, const SysView& s, const SideData& sd, int grid, const double* v,
+                                  double* uh, double* g, double* copies, const double* c0, double* usq, int* done,
+                                  cudaStream_t st) {
+  void (*k)(const CUtensorMap, SysView, int, const double*, const double*, int64_t, double*, double*, double*, int,
+            const double*, double*, int*);
+  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<ATT, true, true> : k_lsqr_fused<ATT, true, false>;
+  else k = p.acc_smem ? k_lsqr_fused<ATT, false, true> : k_lsqr_fused<ATT, false, false>;
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+  if (e != cudaSuccess) return e;
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, sd.xw, sd.xw_axis_stride, uh, g, copies, sd.n_copies, c0,
+                                          usq, done);
+  return cudaGetLastError();
+}
+
+// expand(v) ; fused pass ; [fold instrumental copies into g]
+cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* v,
+                              double* uh, double* g, const double* c0, double* usq, int* done, cudaStream_t st,
+                              int64_t* launches) {
+  if (s.M == 0) return cudaSuccess;
+  const SmemPlan p = plan_smem(s, t, PLAN_FUSED);
+  if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
+  cudaError_t e = launch_expand_att(s, sd, num_sms, v, done, st, launches);
+  if (e != cudaSuccess) return e;
+  const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
+  const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
+  double* copies = use_copies ? sd.ins_copies : nullptr;
+  ++*launches;
+  e = sd.att_mode == ATT_FULL ? launch_fused_t<ATT_FULL>(p, s, sd, grid, v, uh, g, copies, c0, usq, done, st)
+                              : launch_fused_t<ATT_HALF>(p, s, sd, grid, v, uh, g, copies, c0, usq, done, st);
+  if (e != cudaSuccess) return e;
+  if (use_copies) return launch_fold_instr(s, sd, g, done, st, launches);
+  return cudaSuccess;
+}
+
+}  // namespace gsr

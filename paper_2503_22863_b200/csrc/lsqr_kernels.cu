@@ -107,6 +107,30 @@ __global__ void __launch_bounds__(256) k_vscale(double* __restrict__ v, int64_t 
     v[i] *= nb;
 }
 
+// fused path, step 2: beta = ||u_hat||; v <- g / beta - beta v (un-normalised v'), vsq = ||v'||^2.
+// g = A^T u_hat was accumulated by the fused pass.  Thread 0 publishes beta, 1/beta and anorm.
+__global__ void __launch_bounds__(256) k_vcombine(double* __restrict__ v, const double* __restrict__ g, int64_t n,
+                                                  DevScalars* sc) {
+  if (sc->done) return;
+  const double beta = sqrt(sc->usq);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    sc->beta = beta;
+    sc->s_y = beta > 0.0 ? 1.0 / beta : 0.0;
+    if (beta > 0.0) sc->anorm = sqrt(sc->anorm * sc->anorm + sc->alpha * sc->alpha + beta * beta);
+  }
+  if (!(beta > 0.0)) return;                         // P-S: v, alpha unchanged when beta = 0
+  const double ib = 1.0 / beta, nb = -beta;
+  double sq = 0.0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const double t = fma(nb, v[i], g[i] * ib);
+    v[i] = t;
+    sq = fma(t, t, sq);
+  }
+  sq = block_sum(sq);
+  if (threadIdx.x == 0) atomicAdd(&sc->vsq, sq);
+}
+
 // steps 2b-8 of DESIGN.md section 4 (scalars only): alpha, plane rotation, norm estimates, stopping rule
 __global__ void k_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim) {
   if (sc->done) return;
@@ -218,6 +242,10 @@ cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevS
 }
 cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
   k_vscale<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
+  k_vcombine<<<grid_for(n, 256, 4), 256, 0, st>>>(v, g, n, sc);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,

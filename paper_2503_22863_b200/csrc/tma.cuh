@@ -66,8 +66,7 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
       : "memory");
 }
 
-// Per-warp ring of STAGES row tiles.  All 32 lanes call every method; lane 0 talks to the TMA.
-template <int STAGES>
+// Per-warp ring of `nstages` row tiles.  All 32 lanes call every method; lane 0 talks to the TMA.
 struct TileRing {
   char* base;       // this warp's STAGES * STAGE_BYTES of shared memory (128-byte aligned)
   uint64_t* bars;   // this warp's STAGES mbarriers
@@ -77,6 +76,7 @@ struct TileRing {
   int64_t next_issue;           // next tile this warp will request
   uint64_t policy;
   int stage;                    // stage of the next tile to consume
+  int nstages;
   uint32_t phase;
 
   __device__ __forceinline__ void issue(int s, int64_t tile) {
@@ -90,18 +90,18 @@ struct TileRing {
   }
 
   __device__ __forceinline__ void init(char* smem_base, uint64_t* bar_base, const CUtensorMap* m, const int32_t* idx_,
-                                       int64_t M_, int64_t first_tile, int64_t stride_, int lane) {
-    base = smem_base; bars = bar_base; map = m; idx = idx_; M = M_;
+                                       int64_t M_, int64_t first_tile, int64_t stride_, int lane, int nstages_) {
+    base = smem_base; bars = bar_base; map = m; idx = idx_; M = M_; nstages = nstages_;
     n_tiles = (M_ + TILE_ROWS - 1) / TILE_ROWS;
     stride = stride_; next_issue = first_tile; stage = 0; phase = 0;
     policy = l2_policy_evict_first();
     if (lane == 0) {
-      for (int s = 0; s < STAGES; s++) mbar_init(bars + s, 1);
+      for (int s = 0; s < nstages; s++) mbar_init(bars + s, 1);
       mbar_fence_init();
     }
     __syncwarp();
     if (lane == 0) {
-      for (int s = 0; s < STAGES; s++) {
+      for (int s = 0; s < nstages; s++) {
         if (next_issue < n_tiles) issue(s, next_issue);
         next_issue += stride;
       }
@@ -119,7 +119,7 @@ struct TileRing {
     __syncwarp();
     if (lane == 0 && next_issue < n_tiles) issue(stage, next_issue);
     next_issue += stride;
-    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    if (++stage == nstages) { stage = 0; phase ^= 1; }
   }
 };
 

@@ -343,7 +343,7 @@ def test_lsqr_host_entry_matches_device_entry():
         x = torch.empty(C1.n_unknowns, dtype=torch.float64, device=DEV)
         rd = s.lsqr(dev(b), x, 50)
         n0 = s.launch_count()
-        assert n0 > 50 * 6
+        assert n0 >= 50 * 5          # >= 5 kernels per LSQR iteration, all from libgsr
     assert rh.istop == rd.istop == 7 and rh.itn == rd.itn == 50
     assert np.linalg.norm(xh - x.cpu().numpy()) <= 1e-6 * np.linalg.norm(xh)   # (atomics reorder: R16)
     assert abs(rh.bnorm - rd.bnorm) <= 1e-14 * rd.bnorm
