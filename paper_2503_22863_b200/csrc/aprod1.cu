@@ -40,7 +40,9 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const bool valid = r < s.M;
     const double yin = valid ? y[r] : 0.0;
     const char* tile = ring.acquire();
-    const double out = fma(c0, yin, tile_row_dot<ATT, GSMEM>(tile, lane, valid, gc));
+    RowRegs row;
+    load_row(tile, lane, valid, row);
+    const double out = fma(c0, yin, row_dot<ATT, GSMEM>(row, gc));
     if (valid) {
       y[r] = out;
       sq = fma(out, out, sq);
@@ -93,7 +95,8 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   p.gather_smem = p.acc_smem = false;
   const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
   size_t ring = ring_bytes(p.warps, p.stages);
-  size_t left = SMEM_BUDGET > ring ? SMEM_BUDGET - ring : 0;
+  if (ring > SMEM_BUDGET) { p.bytes = ring; return p; }   // caller rejects (cudaErrorInvalidValue)
+  size_t left = SMEM_BUDGET - ring;
   // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1 gathers per row
   if ((what & PLAN_APROD2) && table <= left) { p.acc_smem = true; left -= table; }
   if ((what & PLAN_APROD1) && table <= left) { p.gather_smem = true; left -= table; }

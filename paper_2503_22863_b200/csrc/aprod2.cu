@@ -36,7 +36,10 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const double yv = valid ? ys * y[r] : 0.0;
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     const char* tile = ring.acquire();
-    gacc += tile_scatter<ASMEM>(tile, lane, valid, nvalid, yv, sc);
+    RowRegs row;
+    load_row(tile, lane, valid, row);
+    scatter_att(tile, lane, nvalid, yv, row.i0.y, sc);
+    gacc += scatter_row<ASMEM>(row, lane, valid, yv, sc);
     ring.release(lane);
   }
   if (ASMEM) {

@@ -23,7 +23,33 @@ struct GatherCtx {
   double xg;                // x[oG] (0 when G = 0)
 };
 
-// (A x)[row of this lane]   -- PAPER.md:45, Eq. (2).  Lane-per-row; `valid` = row < M.
+// One row of a staged tile in registers (lane-per-row).
+struct RowRegs {
+  double a[NSLOT];
+  int4 i0, i1;   // {star, att_start, instr0, instr1}, {instr2..5}
+};
+
+// Lane l reads row l of the tile: 12 conflict-free LDS.128 for the coefficients (208-byte stride), and
+// the 32-byte index record as two LDS.128 issued in swizzled order (lanes 4-7, 12-15, ... read the
+// second half first), which makes the 32-byte-stride pattern bank-conflict free.
+// Tail lanes (row >= M) get zero coefficients (TMA zero fill) and an all-zero index record.
+__device__ __forceinline__ void load_row(const char* tile, int lane, bool valid, RowRegs& r) {
+  const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
+#pragma unroll
+  for (int q = 0; q < NSLOT / 2; q++) {
+    const double2 v = ap[q];
+    r.a[2 * q] = v.x;
+    r.a[2 * q + 1] = v.y;
+  }
+  const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
+  const int sw = (lane >> 2) & 1;
+  const int4 first = ip[sw], second = ip[sw ^ 1];
+  r.i0 = sw ? second : first;
+  r.i1 = sw ? first : second;
+  if (!valid) { r.i0 = make_int4(0, 0, 0, 0); r.i1 = r.i0; }
+}
+
+// (A x)[row of this lane]   -- PAPER.md:45, Eq. (2).
 // Gathers (the L1 tag stage serves ~1 random line per cycle per SM, measured 284 G gathers/s
 // chip-wide whatever the access width, so the number of gather instructions per row is what counts):
 //   astro  : x[5*star .. +4]   (rows are sorted by star: the lanes of a warp share 1-2 stars)
@@ -35,30 +61,20 @@ struct GatherCtx {
 //   instr  : shared-memory copy of the instrumental slice when it fits, else L2 gathers
 //   global : one register.
 template <int ATT, bool INSTR_SMEM>
-__device__ __forceinline__ double tile_row_dot(const char* tile, int lane, bool valid, const GatherCtx& c) {
-  const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
-  const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
-  int4 i0 = ip[0], i1 = ip[1];
-  if (!valid) { i0 = make_int4(0, 0, 0, 0); i1 = i0; }   // tail lanes: coefficients are zero-filled by TMA
-  double a[NSLOT];
-#pragma unroll
-  for (int q = 0; q < NSLOT / 2; q++) {
-    const double2 v = ap[q];
-    a[2 * q] = v.x;
-    a[2 * q + 1] = v.y;
-  }
-  const double* xa = c.x + 5 * (int64_t)i0.x;
+__device__ __forceinline__ double row_dot(const RowRegs& r, const GatherCtx& c) {
+  const double* a = r.a;
+  const double* xa = c.x + 5 * (int64_t)r.i0.x;
   double g[NSLOT - 1];
 #pragma unroll
   for (int k = 0; k < 5; k++) g[k] = __ldg(xa + k);
   if (ATT == ATT_FULL) {
-    const double* w0 = c.xw + (int64_t)i0.y * 4;
+    const double* w0 = c.xw + (int64_t)r.i0.y * 4;
     ld_nc_v4(w0, g[5], g[6], g[7], g[8]);
     ld_nc_v4(w0 + c.xw_axis_stride, g[9], g[10], g[11], g[12]);
     ld_nc_v4(w0 + 2 * c.xw_axis_stride, g[13], g[14], g[15], g[16]);
   } else {
-    const bool odd = i0.y & 1;
-    const double* w0 = c.xw + (int64_t)(i0.y >> 1) * 4;
+    const bool odd = r.i0.y & 1;
+    const double* w0 = c.xw + (int64_t)(r.i0.y >> 1) * 4;
 #pragma unroll
     for (int ax = 0; ax < 3; ax++) {
       double e0, e1, e2, e3, f0 = 0.0, f1 = 0.0, f2 = 0.0, f3 = 0.0;
@@ -71,7 +87,7 @@ __device__ __forceinline__ double tile_row_dot(const char* tile, int lane, bool 
     }
   }
   {
-    const int col[6] = {i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+    const int col[6] = {r.i0.z, r.i0.w, r.i1.x, r.i1.y, r.i1.z, r.i1.w};
 #pragma unroll
     for (int q = 0; q < 6; q++) g[17 + q] = INSTR_SMEM ? c.xi_s[col[q]] : __ldg(c.xi_g + col[q]);
   }
@@ -89,7 +105,7 @@ __device__ __forceinline__ double tile_row_dot(const char* tile, int lane, bool 
 
 // Where a kernel scatters to (aprod 2 side).
 struct ScatterCtx {
-  double* x;        // the n-vector being accumulated into (astro and global parts, attitude base)
+  double* x;        // the n-vector being accumulated into (astro and global parts)
   double* xatt;     // x + oA
   double* xins;     // instrumental accumulator in global memory: x + oI, or this CTA's private copy
   double* acc_s;    // shared-memory instrumental accumulator, or nullptr
@@ -98,37 +114,40 @@ struct ScatterCtx {
 
 // x[col(r,k)] += a[r][k] * yv  for the 32 rows of a tile  -- PAPER.md:49, Eq. (3).
 // yv = the lane's (scaled) y value, 0 for tail lanes; nvalid = rows of the tile that exist.
+//
+// Attitude (slots 5-16): the 12 x 32 products are walked so that 4 consecutive lanes cover one
+// 4-knot run: its fp64 reductions then travel to L2 as one request (measured 2.2x the add rate of
+// lane-per-row issue).  Pass `it` handles axis it%3 of rows 8*(it/3) .. +7; each half-warp takes the
+// rows of one parity (r, r+2, r+4, r+6): with the 208-byte row stride their 32-byte runs fall in
+// disjoint banks, so the LDS.64 is conflict free.  att_start and y come by shuffle from the lane that
+// owns the row.
+__device__ __forceinline__ void scatter_att(const char* tile, int lane, int nvalid, double yv, int att_start,
+                                            const ScatterCtx& c) {
+  const double* td = reinterpret_cast<const double*>(tile);
+  const int sub = 2 * ((lane >> 2) & 3) + (lane >> 4);   // row within the group of 8
+  const int j = lane & 3;
+#pragma unroll
+  for (int it = 0; it < 12; it++) {
+    const int ax = it % 3, row = 8 * (it / 3) + sub;
+    const double yy = __shfl_sync(0xffffffffu, yv, row);
+    const int att = __shfl_sync(0xffffffffu, att_start, row);
+    if (row < nvalid) {
+      const double a = td[row * ROW_STRIDE_D + 5 + 4 * ax + j];
+      atomicAdd(c.xatt + (int64_t)ax * c.K + att + j, a * yy);
+    }
+  }
+}
+
+// Astrometric, instrumental and global slots of the lane's own row, from registers.
 //  astro  (slots 0-4)  : rows are sorted by star, so the lanes of a warp hold runs of equal star; a
 //                        segmented warp scan (shuffles) sums each run, the run head issues 5 adds.
-//  att    (slots 5-16) : the 12 x 32 products are walked element-per-lane, so 4 consecutive lanes
-//                        cover one 4-knot run and its fp64 reductions travel to L2 as one request
-//                        (measured 2.2x the add rate of lane-per-row issue).
 //  instr  (slots 17-22): block-privatised accumulators in shared memory when the slice fits (flushed
 //                        once per CTA), else reductions at L2.
 //  global (slot 23)    : returned as the lane's contribution, reduced once per CTA by the caller.
 template <bool INSTR_SMEM>
-__device__ __forceinline__ double tile_scatter(const char* tile, int lane, bool valid, int nvalid, double yv,
-                                               const ScatterCtx& c) {
-  const double* td = reinterpret_cast<const double*>(tile);
-  const int32_t* ti = reinterpret_cast<const int32_t*>(tile + COEF_TILE_BYTES);
-#pragma unroll
-  for (int it = 0; it < 12; it++) {
-    const int e = it * 32 + lane;
-    const int row = e / 12, sl = e - row * 12;
-    const double yy = __shfl_sync(0xffffffffu, yv, row);
-    if (row < nvalid) {
-      const double a = td[row * ROW_STRIDE_D + 5 + sl];
-      const int att = ti[row * 8 + 1];
-      atomicAdd(c.xatt + (int64_t)(sl >> 2) * c.K + att + (sl & 3), a * yy);
-    }
-  }
-  const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
-  const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
-  const int4 i0 = ip[0], i1 = ip[1];
-  const double2 a01 = ap[0], a23 = ap[1], a45 = ap[2];
-  const double2 a1617 = ap[8], a1819 = ap[9], a2021 = ap[10], a2223 = ap[11];
-  const int star = valid ? i0.x : (-1 - lane);
-  double p0 = a01.x * yv, p1 = a01.y * yv, p2 = a23.x * yv, p3 = a23.y * yv, p4 = a45.x * yv;
+__device__ __forceinline__ double scatter_row(const RowRegs& r, int lane, bool valid, double yv, const ScatterCtx& c) {
+  const int star = valid ? r.i0.x : (-1 - lane);
+  double p0 = r.a[0] * yv, p1 = r.a[1] * yv, p2 = r.a[2] * yv, p3 = r.a[3] * yv, p4 = r.a[4] * yv;
 #pragma unroll
   for (int off = 1; off < 32; off <<= 1) {
     const int so = __shfl_down_sync(0xffffffffu, star, off);
@@ -144,12 +163,10 @@ __device__ __forceinline__ double tile_scatter(const char* tile, int lane, bool 
   }
   double gl = 0.0;
   if (valid) {
-    const double v17 = a1617.y * yv, v18 = a1819.x * yv, v19 = a1819.y * yv, v20 = a2021.x * yv,
-                 v21 = a2021.y * yv, v22 = a2223.x * yv;
     double* t = INSTR_SMEM ? c.acc_s : c.xins;
-    atomicAdd(t + i0.z, v17); atomicAdd(t + i0.w, v18); atomicAdd(t + i1.x, v19);
-    atomicAdd(t + i1.y, v20); atomicAdd(t + i1.z, v21); atomicAdd(t + i1.w, v22);
-    gl = a2223.y * yv;
+    atomicAdd(t + r.i0.z, r.a[17] * yv); atomicAdd(t + r.i0.w, r.a[18] * yv); atomicAdd(t + r.i1.x, r.a[19] * yv);
+    atomicAdd(t + r.i1.y, r.a[20] * yv); atomicAdd(t + r.i1.z, r.a[21] * yv); atomicAdd(t + r.i1.w, r.a[22] * yv);
+    gl = r.a[23] * yv;
   }
   return gl;
 }

@@ -53,14 +53,17 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const double uin = valid ? uh[r] : 0.0;
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     const char* tile = ring.acquire();
-    double out = fma(c0, uin, tile_row_dot<ATT, GSMEM>(tile, lane, valid, gc));
+    RowRegs row;
+    load_row(tile, lane, valid, row);
+    double out = fma(c0, uin, row_dot<ATT, GSMEM>(row, gc));
     if (valid) {
       uh[r] = out;
       sq = fma(out, out, sq);
     } else {
       out = 0.0;
     }
-    gacc += tile_scatter<ASMEM>(tile, lane, valid, nvalid, out, sc);
+    scatter_att(tile, lane, nvalid, out, row.i0.y, sc);
+    gacc += scatter_row<ASMEM>(row, lane, valid, out, sc);
     ring.release(lane);
   }
   if (ASMEM) {
