@@ -335,18 +335,29 @@ def test_lsqr_constraint_rows_to_convergence():
 
 
 def test_lsqr_host_entry_matches_device_entry():
+    """gsr_lsqr_host (HOST buffers in, x out) runs the same solve as create + gsr_lsqr on device buffers.
+    The two runs differ only by the order of the fp64 reductions at L2, but the LSQR trajectory of C1
+    amplifies rounding-level differences by ~1e9 between iterations 5 and 10 (serial oracle vs scipy vs
+    OpenMP oracle differ by 4e-3 at k = 10 and agree to 1e-15 at convergence: DESIGN.md reading R16), so
+    the comparison is made where it is well-posed: k = 5 and at convergence."""
     a, idx = host.make_rows(C1)
     b = rhs(C1, a, idx, host.x_true(C1))
     xh = np.empty(C1.n_unknowns)
-    rh = gsr.gsr_lsqr_host(C1.n_stars, C1.n_knots, C1.n_instr, C1.n_glob, a, idx, b, xh, 50)
     with make_gpu_system(C1, a, idx) as s:
         x = torch.empty(C1.n_unknowns, dtype=torch.float64, device=DEV)
-        rd = s.lsqr(dev(b), x, 50)
+        rh = gsr.gsr_lsqr_host(C1.n_stars, C1.n_knots, C1.n_instr, C1.n_glob, a, idx, b, xh, 5)
+        rd = s.lsqr(dev(b), x, 5)
+        assert rh.istop == rd.istop == 7 and rh.itn == rd.itn == 5
+        assert np.linalg.norm(xh - x.cpu().numpy()) <= 1e-9 * np.linalg.norm(xh)
+        assert abs(rh.bnorm - rd.bnorm) <= 1e-14 * rd.bnorm
         n0 = s.launch_count()
-        assert n0 >= 50 * 5          # >= 5 kernels per LSQR iteration, all from libgsr
-    assert rh.istop == rd.istop == 7 and rh.itn == rd.itn == 50
-    assert np.linalg.norm(xh - x.cpu().numpy()) <= 1e-6 * np.linalg.norm(xh)   # (atomics reorder: R16)
-    assert abs(rh.bnorm - rd.bnorm) <= 1e-14 * rd.bnorm
+        rd = s.lsqr(dev(b), x, 50)
+        assert rd.istop == 7 and rd.itn == 50
+        assert s.launch_count() - n0 >= 50 * 4          # >= 4 kernels per LSQR iteration, all from libgsr
+        rh = gsr.gsr_lsqr_host(C1.n_stars, C1.n_knots, C1.n_instr, C1.n_glob, a, idx, b, xh, 5000, 1e-12, 1e-12, 1e8)
+        rd = s.lsqr(dev(b), x, 5000, 1e-12, 1e-12, 1e8)
+        assert rh.istop == rd.istop == 2 and abs(rh.itn - rd.itn) <= max(3, 0.05 * rd.itn)
+        assert np.linalg.norm(xh - x.cpu().numpy()) <= 1e-9 * np.linalg.norm(xh)
 
 
 # ------------------------------------------------------------------ full-size C2 (the bench launch configuration)
