@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--oracle-rows", type=int, default=0, help="rows of the oracle sample (0 = auto)")
     ap.add_argument("--option", action="append", default=[], help="name=value passed to gsr_set_option")
+    ap.add_argument("--stars", type=int, default=0,
+                    help="profiling aid: same workload family with this many stars (K, I unchanged); 0 = the config's")
     return ap.parse_args()
 
 
@@ -243,6 +245,8 @@ def run_gsr(args):
         dist.init_process_group("nccl", device_id=dev)
     free, total = torch.cuda.mem_get_info()
     shape = pick_workload(args.workload, free)
+    if args.stars > 0:
+        shape = shape.scaled(args.stars, name=f"{shape.name}[{args.stars} stars]")
     K, W = args.steps, max(args.warmup, 3)
 
     vals, idx = gdev.make_system(shape, device=dev)

@@ -4,12 +4,12 @@
 
 namespace gsr {
 
-// ---- variant 1 (default): TMA-staged row tiles, one warp per tile, lane per row -----------------
-template <int ATT, bool GSMEM>
-__global__ void __launch_bounds__(512, 1)
+// ---- variant 1 (default): TMA-staged row tiles, one warp per tile ---------------------------------
+template <bool GSMEM>
+__global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ x,
-             const double* __restrict__ xw, int64_t xw_axis_stride, double* __restrict__ y,
-             const double* __restrict__ c0p, double* sumsq, int* done) {
+             const double* __restrict__ att_il, double* __restrict__ y, const double* __restrict__ c0p, double* sumsq,
+             int* done) {
   if (done) {
     const int d = *done;
     if (d) {  // LSQR already stopped: no-op (and latch "update pending" 2 -> 1, see k_step_scalars)
@@ -31,18 +31,24 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(x + s.oI + i);
     __syncthreads();
   }
-  GatherCtx gc{x, xw, xw_axis_stride, xi_s, x + s.oI, s.G ? __ldg(x + s.oG) : 0.0};
+  GatherCtx gc{x, att_il, xi_s, x + s.oI, s.G ? __ldg(x + s.oG) : 0.0};
+  const AttLane al(lane);
   const double c0 = c0p ? *c0p : 1.0;
   double sq = 0.0;
 
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
-    const int64_t r = t * TILE_ROWS + lane;
+    const int64_t row0 = t * TILE_ROWS;
+    const int64_t r = row0 + lane;
     const bool valid = r < s.M;
+    const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     const double yin = valid ? y[r] : 0.0;
     const char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    const double out = fma(c0, yin, row_dot<ATT, GSMEM>(row, gc));
+    double c[16];
+    att_load_coefs(tile, al, nvalid, c);
+    const double dot = att_dot(al, lane, nvalid, row.i0.y, att_il, c) + row_dot_rest<GSMEM>(row, gc);
+    const double out = fma(c0, yin, dot);
     if (valid) {
       y[r] = out;
       sq = fma(out, out, sq);
@@ -55,32 +61,55 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   }
 }
 
-// Expanded attitude windows, rebuilt from x before every gather pass (3K reads, <= 12K writes: << matrix).
-//   step 1 (ATT_FULL): xw[(ax*nwin + t)*4 + j] = x[oA + ax*K + t + j],  t = 0 .. K-4
-//   step 2 (ATT_HALF): xw[(ax*nwin + w)*4 + j] = x[oA + ax*K + 2w + j], w = 0 .. (K-2)/2
-// Elements past the end of x (only pad slots of the very last windows) read as 0.
-__global__ void __launch_bounds__(256) k_expand_att(const double* __restrict__ x, int64_t oA, int64_t n, int64_t K,
-                                                    int step, int64_t nwin, double* __restrict__ xw, const int* done) {
+// Attitude block between the API layout (axis-major: x[oA + ax*K + t]) and the interleaved layout the
+// kernels gather from / scatter into (il[3*t + ax]); 3K elements, negligible next to the matrix.
+__global__ void __launch_bounds__(256) k_att_to_il(const double* __restrict__ xatt, int64_t K, double* __restrict__ il,
+                                                   const int* done) {
   if (done && *done) return;
-  const int64_t total = 3 * nwin;
+  const int64_t total = 3 * K;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t ax = i / nwin, w = i - ax * nwin;
-    const int64_t e = oA + ax * K + w * step;
-    double v[4];
-#pragma unroll
-    for (int j = 0; j < 4; j++) v[j] = (e + j < n) ? __ldg(x + e + j) : 0.0;
-    double2* o = reinterpret_cast<double2*>(xw + i * 4);
-    o[0] = make_double2(v[0], v[1]);
-    o[1] = make_double2(v[2], v[3]);
+    const int64_t t = i / 3, ax = i - 3 * t;
+    il[i] = __ldg(xatt + ax * K + t);
+  }
+}
+// x_att[ax*K + t] += il[3*t + ax] ; il <- 0   (folds the interleaved accumulator of a standalone aprod 2)
+__global__ void __launch_bounds__(256) k_att_fold(double* __restrict__ xatt, int64_t K, double* __restrict__ il) {
+  const int64_t total = 3 * K;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t ax = i / K, t = i - ax * K;
+    xatt[i] += il[3 * t + ax];
+  }
+}
+// dst[ax*K + t] = il[3*t + ax]   (export of an internal n-vector's attitude block)
+__global__ void __launch_bounds__(256) k_att_from_il(const double* __restrict__ il, int64_t K, double* __restrict__ dst) {
+  const int64_t total = 3 * K;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t ax = i / K, t = i - ax * K;
+    dst[i] = il[3 * t + ax];
   }
 }
 
-cudaError_t launch_expand_att(const SysView& s, const SideData& sd, int num_sms, const double* x, const int* done,
-                              cudaStream_t st, int64_t* launches) {
-  const int64_t total = 3 * sd.xw_nwin;
-  int64_t eb = (total + 255) / 256;
-  if (eb > num_sms * 8) eb = num_sms * 8;
-  k_expand_att<<<(unsigned)eb, 256, 0, st>>>(x, s.oA, s.n, s.K, sd.att_mode == ATT_FULL ? 1 : 2, sd.xw_nwin, sd.xw, done);
+static unsigned att_grid(int64_t K, int num_sms) {
+  int64_t b = (3 * K + 255) / 256;
+  if (b > (int64_t)num_sms * 8) b = (int64_t)num_sms * 8;
+  return (unsigned)(b < 1 ? 1 : b);
+}
+cudaError_t launch_att_to_il(const SysView& s, int num_sms, const double* x_std, double* il, const int* done,
+                             cudaStream_t st, int64_t* launches) {
+  k_att_to_il<<<att_grid(s.K, num_sms), 256, 0, st>>>(x_std + s.oA, s.K, il, done);
+  ++*launches;
+  return cudaGetLastError();
+}
+cudaError_t launch_att_fold(const SysView& s, int num_sms, double* x_std, double* il, cudaStream_t st, int64_t* launches) {
+  k_att_fold<<<att_grid(s.K, num_sms), 256, 0, st>>>(x_std + s.oA, s.K, il);
+  ++*launches;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  return cudaMemsetAsync(il, 0, (size_t)(3 * s.K) * sizeof(double), st);
+}
+cudaError_t launch_att_from_il(const SysView& s, int num_sms, const double* il, double* dst_std_att, cudaStream_t st,
+                               int64_t* launches) {
+  k_att_from_il<<<att_grid(s.K, num_sms), 256, 0, st>>>(il, s.K, dst_std_att);
   ++*launches;
   return cudaGetLastError();
 }
@@ -90,7 +119,7 @@ static size_t ring_bytes(int w, int st) { return (size_t)w * st * STAGE_BYTES + 
 
 SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   SmemPlan p;
-  p.warps = t.warps > 0 ? t.warps : 8;
+  p.warps = t.warps > 0 ? t.warps : 12;
   p.stages = t.stages > 0 ? t.stages : 2;
   p.gather_smem = p.acc_smem = false;
   const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
@@ -104,18 +133,18 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   return p;
 }
 
-template <int ATT>
 static cudaError_t launch_tma1(bool gsmem, const SysView& s, const SideData& sd, int grid, const SmemPlan& p,
-                               const double* x, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st) {
-  auto k = gsmem ? k_aprod1_tma<ATT, true> : k_aprod1_tma<ATT, false>;
+                               const double* x, const double* att_il, double* y, const double* c0, double* sumsq,
+                               int* done, cudaStream_t st) {
+  auto k = gsmem ? k_aprod1_tma<true> : k_aprod1_tma<false>;
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
   if (e != cudaSuccess) return e;
-  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, x, sd.xw, sd.xw_axis_stride, y, c0, sumsq, done);
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, x, att_il, y, c0, sumsq, done);
   return cudaGetLastError();
 }
 
 // ---- variant 0: one thread per row, direct global loads (simple device-side cross-check) --------
-__global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const double* __restrict__ x,
+__global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const double* __restrict__ x, bool x_il,
                                                           double* __restrict__ y,
                                                           const double* __restrict__ c0p,
                                                           double* sumsq, int* done) {
@@ -144,11 +173,12 @@ __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const doubl
     double acc = 0.0;
 #pragma unroll
     for (int k = 0; k < 5; k++) acc = fma(a[k], __ldg(xa + k), acc);
-    const double* xt = x + s.oA + i0.y;
+    const int64_t sa = x_il ? 1 : s.K, sj = x_il ? 3 : 1;   // attitude strides: axis, knot
+    const double* xt = x + s.oA + i0.y * sj;
 #pragma unroll
     for (int ax = 0; ax < 3; ax++)
 #pragma unroll
-      for (int j = 0; j < 4; j++) acc = fma(a[5 + 4 * ax + j], __ldg(xt + ax * s.K + j), acc);
+      for (int j = 0; j < 4; j++) acc = fma(a[5 + 4 * ax + j], __ldg(xt + ax * sa + j * sj), acc);
     const double* xi = x + s.oI;
     acc = fma(a[17], __ldg(xi + i0.z), acc);
     acc = fma(a[18], __ldg(xi + i0.w), acc);
@@ -167,25 +197,30 @@ __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const doubl
   }
 }
 
+// x_il = true: the attitude block of x is already interleaved (LSQR-internal vectors); otherwise x is in
+// the API layout and its attitude block is first copied into the side buffer sd.att_il.
 cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* x,
-                          double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
+                          bool x_il, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
   if (t.aprod1_variant == 1) {
     const SmemPlan p = plan_smem(s, t, PLAN_APROD1);
-    if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
-    cudaError_t e = launch_expand_att(s, sd, num_sms, x, done, st, launches);
-    if (e != cudaSuccess) return e;
+    if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
+    const double* att_il = x + s.oA;
+    if (!x_il) {
+      cudaError_t e = launch_att_to_il(s, num_sms, x, sd.att_il, done, st, launches);
+      if (e != cudaSuccess) return e;
+      att_il = sd.att_il;
+    }
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
     ++*launches;
-    return sd.att_mode == ATT_FULL ? launch_tma1<ATT_FULL>(p.gather_smem, s, sd, grid, p, x, y, c0, sumsq, done, st)
-                                   : launch_tma1<ATT_HALF>(p.gather_smem, s, sd, grid, p, x, y, c0, sumsq, done, st);
+    return launch_tma1(p.gather_smem, s, sd, grid, p, x, att_il, y, c0, sumsq, done, st);
   }
   const int threads = 256;
   int64_t blocks = (s.M + threads - 1) / threads;
   const int64_t cap = (int64_t)num_sms * 8;
   if (blocks > cap) blocks = cap;
-  k_aprod1_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, x, y, c0, sumsq, done);
+  k_aprod1_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, x, x_il, y, c0, sumsq, done);
   ++*launches;
   return cudaGetLastError();
 }

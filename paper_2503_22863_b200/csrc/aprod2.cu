@@ -3,12 +3,12 @@
 
 namespace gsr {
 
-// ---- variant 1 (default): TMA-staged row tiles, split by parameter block (tile_scatter) ---------
+// ---- variant 1 (default): TMA-staged row tiles, split by parameter block (aprod_device.cuh) ------
 template <bool ASMEM>
-__global__ void __launch_bounds__(512, 1)
+__global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
-             double* __restrict__ x, double* ins_copies, int n_copies, const double* __restrict__ yscale,
-             const int* done) {
+             double* __restrict__ x, double* __restrict__ gatt_il, double* ins_copies, int n_copies,
+             const double* __restrict__ yscale, const int* done) {
   if (done && *done) return;
   extern __shared__ char smem_raw[];
   char* smem = smem_align128(smem_raw);
@@ -24,8 +24,9 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
     __syncthreads();
   }
-  ScatterCtx sc{x, x + s.oA, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : x + s.oI,
-                acc_s, s.K};
+  ScatterCtx sc{x, gatt_il, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : x + s.oI,
+                acc_s};
+  const AttLane al(lane);
   const double ys = yscale ? *yscale : 1.0;
   double gacc = 0.0;
 
@@ -38,7 +39,9 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    scatter_att(tile, lane, nvalid, yv, row.i0.y, sc);
+    double c[16];
+    att_load_coefs(tile, al, nvalid, c);
+    att_scatter(al, nvalid, yv, row.i0.y, gatt_il, c);
     gacc += scatter_row<ASMEM>(row, lane, valid, yv, sc);
     ring.release(lane);
   }
@@ -83,7 +86,7 @@ cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, c
 
 // ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check) ----
 __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const double* __restrict__ y,
-                                                          double* __restrict__ x,
+                                                          double* __restrict__ x, bool x_il,
                                                           const double* __restrict__ yscale,
                                                           const int* done) {
   if (done && *done) return;
@@ -106,11 +109,12 @@ __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const doubl
       double* xa = x + 5 * (int64_t)i0.x;
 #pragma unroll
       for (int k = 0; k < 5; k++) atomicAdd(xa + k, a[k] * yr);
-      double* xt = x + s.oA + i0.y;
+      const int64_t sa = x_il ? 1 : s.K, sj = x_il ? 3 : 1;   // attitude strides: axis, knot
+      double* xt = x + s.oA + i0.y * sj;
 #pragma unroll
       for (int ax = 0; ax < 3; ax++)
 #pragma unroll
-        for (int j = 0; j < 4; j++) atomicAdd(xt + ax * s.K + j, a[5 + 4 * ax + j] * yr);
+        for (int j = 0; j < 4; j++) atomicAdd(xt + ax * sa + j * sj, a[5 + 4 * ax + j] * yr);
       double* xi = x + s.oI;
       atomicAdd(xi + i0.z, a[17] * yr);
       atomicAdd(xi + i0.w, a[18] * yr);
@@ -127,22 +131,29 @@ __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const doubl
   }
 }
 
+// x_il = true: x is an LSQR-internal vector (attitude block interleaved) and is scattered into directly;
+// otherwise the attitude products go to the zeroed side buffer sd.att_acc and are folded into x.
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
-                          double* x, const double* yscale, const int* done, cudaStream_t st, int64_t* launches) {
+                          double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
+                          int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
   if (t.aprod2_variant == 1) {
     const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
-    if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
+    if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
     auto k = p.acc_smem ? k_aprod2_tma<true> : k_aprod2_tma<false>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
     const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
-    k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, use_copies ? sd.ins_copies : nullptr, sd.n_copies,
-                                            yscale, done);
+    k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc,
+                                            use_copies ? sd.ins_copies : nullptr, sd.n_copies, yscale, done);
     ++*launches;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (!x_il) {   // (never inside LSQR, so no `done` gate is needed)
+      e = launch_att_fold(s, num_sms, x, sd.att_acc, st, launches);
+      if (e != cudaSuccess) return e;
+    }
     if (use_copies) return launch_fold_instr(s, sd, x, done, st, launches);
     return cudaSuccess;
   }
@@ -150,7 +161,7 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
   int64_t blocks = (s.M + threads - 1) / threads;
   const int64_t cap = (int64_t)num_sms * 8;
   if (blocks > cap) blocks = cap;
-  k_aprod2_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, y, x, yscale, done);
+  k_aprod2_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, y, x, x_il, yscale, done);
   ++*launches;
   return cudaGetLastError();
 }

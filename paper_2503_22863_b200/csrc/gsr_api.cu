@@ -89,19 +89,15 @@ static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M
   return GSR_OK;
 }
 
-// (Re)allocate the expanded attitude-window table for the requested mode (0 = choose by size).
-static int build_att_table(gsr_system* s, int mode) {
-  const SysView& v = s->v;
-  const size_t full_bytes = (size_t)(3 * (v.K - 3)) * 32;
-  if (mode == 0) mode = full_bytes <= ATT_FULL_MAX_BYTES ? 1 : 2;
-  const int64_t nwin = mode == 1 ? v.K - 3 : (v.K - 2) / 2 + 1;
-  cudaFree(s->side.xw);
-  s->side.xw = nullptr;
-  cudaError_t e = cudaMalloc(&s->side.xw, (size_t)(3 * nwin * 4) * sizeof(double));
-  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc xw"); }
-  s->side.att_mode = mode;
-  s->side.xw_nwin = nwin;
-  s->side.xw_axis_stride = 4 * nwin;
+// Side buffers for the standalone products: the attitude block in the interleaved layout (aprod 1 input
+// copy, aprod 2 accumulator).  LSQR-internal vectors are interleaved already and do not use them.
+static int build_att_buffers(gsr_system* s) {
+  const size_t bytes = (size_t)(3 * s->v.K) * sizeof(double);
+  cudaError_t e = cudaMalloc(&s->side.att_il, bytes);
+  if (e == cudaSuccess) e = cudaMalloc(&s->side.att_acc, bytes);
+  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc att"); }
+  e = cudaMemset(s->side.att_acc, 0, bytes);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaMemset att_acc");
   return GSR_OK;
 }
 
@@ -153,12 +149,12 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
   cudaFree(flag);
   if (e != cudaSuccess) { delete s; return cuda_fail(e, "gsr_create validation"); }
   if (h != 0) { delete s; return GSR_ELAYOUT; }
-  // side structures: the row-tile tensor map and the expanded attitude-window table
+  // side structures: the row-tile tensor map, the interleaved attitude buffers, instrumental replicas
   if (v.M > 0) {
     int rc = make_row_tensor_map(&s->side.map, values, v.M);
     if (rc) { delete s; return rc; }
   }
-  int rc2 = build_att_table(s, 0);
+  int rc2 = build_att_buffers(s);
   if (rc2 == GSR_OK) rc2 = build_instr_copies(s);
   if (rc2) { gsr_destroy(s); return rc2; }
   *out = s;
@@ -175,7 +171,7 @@ static void free_events(gsr_system* s) {
 extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
-  cudaFree(s->side.xw); cudaFree(s->side.ins_copies); cudaFree(s->g);
+  cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins_copies); cudaFree(s->g);
   free_events(s);
   delete s;
 }
@@ -204,20 +200,20 @@ static void prof_end(gsr_system* s, cudaStream_t st, EventPair* ep) {
   s->pending.push_back(*ep);
 }
 
-static int do_aprod1(gsr_system* s, const double* x, double* y, const double* c0, double* sumsq,
+static int do_aprod1(gsr_system* s, const double* x, bool x_il, double* y, const double* c0, double* sumsq,
                      int* done, cudaStream_t st) {
   EventPair ep;
   const bool p = prof_begin(s, 1, st, &ep);
-  cudaError_t e = launch_aprod1(s->v, s->side, s->tune, s->num_sms, x, y, c0, sumsq, done, st, &s->launches);
+  cudaError_t e = launch_aprod1(s->v, s->side, s->tune, s->num_sms, x, x_il, y, c0, sumsq, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod1 launch");
   return GSR_OK;
 }
-static int do_aprod2(gsr_system* s, const double* y, double* x, const double* yscale, const int* done,
+static int do_aprod2(gsr_system* s, const double* y, double* x, bool x_il, const double* yscale, const int* done,
                      cudaStream_t st) {
   EventPair ep;
   const bool p = prof_begin(s, 2, st, &ep);
-  cudaError_t e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, yscale, done, st, &s->launches);
+  cudaError_t e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, x_il, yscale, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod2 launch");
   return GSR_OK;
@@ -225,11 +221,11 @@ static int do_aprod2(gsr_system* s, const double* y, double* x, const double* ys
 
 extern "C" int gsr_aprod1(gsr_system* s, const double* x, double* y, void* stream) {
   if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
-  return do_aprod1(s, x, y, nullptr, nullptr, nullptr, S(stream));
+  return do_aprod1(s, x, false, y, nullptr, nullptr, nullptr, S(stream));
 }
 extern "C" int gsr_aprod2(gsr_system* s, const double* y, double* x, void* stream) {
   if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
-  return do_aprod2(s, y, x, nullptr, nullptr, S(stream));
+  return do_aprod2(s, y, x, false, nullptr, nullptr, S(stream));
 }
 
 // ---- LSQR ------------------------------------------------------------------------------------
@@ -261,7 +257,7 @@ extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
   CU(cudaMemsetAsync(s->vv, 0, (size_t)n * sizeof(double), st));
   CU(lsqr_launch_init_u(b, s->u, M, s->sc, st, &s->launches));           // u_hat = b, usq
   CU(lsqr_launch_init_s1(s->sc, st, &s->launches));                      // beta
-  rc = do_aprod2(s, s->u, s->vv, &s->sc->s_y, nullptr, st);              // v = A^T u
+  rc = do_aprod2(s, s->u, s->vv, true, &s->sc->s_y, nullptr, st);        // v = A^T u
   if (rc) return rc;
   CU(lsqr_launch_sumsq_v(s->vv, n, s->sc, st, &s->launches));
   CU(lsqr_launch_init_s2(s->sc, st, &s->launches));                      // alpha and the rest
@@ -294,17 +290,26 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
   }
   for (int64_t it = 0; it < n_iters && !s->tune.fused; ++it) {
     // 1: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2              (aprod 1)
-    int rc = do_aprod1(s, s->vv, s->u, &sc->c0_u, &sc->usq, &sc->done, st);
+    int rc = do_aprod1(s, s->vv, true, s->u, &sc->c0_u, &sc->usq, &sc->done, st);
     if (rc) return rc;
     // 2: beta ; v <- -beta v ; v += A^T (u_hat / beta) ; vsq = ||v||^2      (aprod 2)
     CU(lsqr_launch_vscale(s->vv, n, sc, st, &s->launches));
-    rc = do_aprod2(s, s->u, s->vv, &sc->s_y, &sc->done, st);
+    rc = do_aprod2(s, s->u, s->vv, true, &sc->s_y, &sc->done, st);
     if (rc) return rc;
     CU(lsqr_launch_sumsq_v(s->vv, n, sc, st, &s->launches));
     // 3-8: scalars, stopping rule ; then the x / w / v update
     CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
     CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, st, &s->launches));
   }
+  return GSR_OK;
+}
+
+// Copy an LSQR-internal n-vector (attitude block interleaved) to a caller's vector in the API layout.
+static int export_nvec(gsr_system* s, const double* src, double* dst, cudaStream_t st) {
+  const SysView& v = s->v;
+  CU(cudaMemcpyAsync(dst, src, (size_t)v.oA * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  CU(launch_att_from_il(v, s->num_sms, src + v.oA, dst + v.oA, st, &s->launches));
+  CU(cudaMemcpyAsync(dst + v.oI, src + v.oI, (size_t)(v.n - v.oI) * sizeof(double), cudaMemcpyDeviceToDevice, st));
   return GSR_OK;
 }
 
@@ -325,9 +330,10 @@ extern "C" int gsr_lsqr_result_get(gsr_system* s, double* x_out, gsr_lsqr_result
   if (!s || !res) return GSR_EINVAL;
   if (!s->lsqr_ready) return GSR_ESTATE;
   cudaStream_t st = S(stream);
-  if (x_out) CU(cudaMemcpyAsync(x_out, s->x, (size_t)s->v.n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  int rc;
+  if (x_out && (rc = export_nvec(s, s->x, x_out, st))) return rc;
   DevScalars h;
-  int rc = fetch_scalars(s, &h, st);
+  rc = fetch_scalars(s, &h, st);
   if (rc) return rc;
   fill_result(h, res);
   return GSR_OK;
@@ -338,13 +344,13 @@ extern "C" int gsr_lsqr_get_state(gsr_system* s, double* u, double* v, double* w
   if (!s) return GSR_EINVAL;
   if (!s->lsqr_ready) return GSR_ESTATE;
   cudaStream_t st = S(stream);
-  const size_t nb = (size_t)s->v.n * sizeof(double);
+  int rc;
   if (u && s->v.M > 0) CU(lsqr_launch_export_u(s->u, u, s->v.M, s->sc, st, &s->launches));
-  if (v) CU(cudaMemcpyAsync(v, s->vv, nb, cudaMemcpyDeviceToDevice, st));
-  if (w) CU(cudaMemcpyAsync(w, s->w, nb, cudaMemcpyDeviceToDevice, st));
-  if (x) CU(cudaMemcpyAsync(x, s->x, nb, cudaMemcpyDeviceToDevice, st));
+  if (v && (rc = export_nvec(s, s->vv, v, st))) return rc;
+  if (w && (rc = export_nvec(s, s->w, w, st))) return rc;
+  if (x && (rc = export_nvec(s, s->x, x, st))) return rc;
   DevScalars h;
-  int rc = fetch_scalars(s, &h, st);
+  rc = fetch_scalars(s, &h, st);
   if (rc) return rc;
   if (out) {
     out->itn = h.itn; out->istop = h.istop;
@@ -466,11 +472,6 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "stages")) s->tune.stages = (int)value;
   else if (!strcmp(name, "instr_copies")) s->tune.instr_copies = (int)value;
   else if (!strcmp(name, "fused")) s->tune.fused = (int)value;
-  else if (!strcmp(name, "att_mode")) {
-    if (value < 0 || value > 2) return GSR_EINVAL;
-    cudaDeviceSynchronize();
-    return build_att_table(s, (int)value);
-  }
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;
   else return GSR_EINVAL;
   return GSR_OK;

@@ -42,38 +42,40 @@ struct Tuning {
   int check_every = 16;    // LSQR iterations between host polls of the stop flag
   int instr_copies = 1;    // replicate the instrumental accumulator in global memory when it cannot be privatised
   int fused = 1;           // LSQR: one fused pass over the matrix per iteration (lsqr_fused.cu)
-  int att_mode = 0;        // 0 = auto (by table size), 1 = full expansion, 2 = half expansion
 };
 
 // Side structures owned by the library (built in gsr_create).
 struct SideData {
   CUtensorMap map;         // 24 x M fp64 tensor, box 26 x 32 (tma.cuh)
-  double* xw = nullptr;    // expanded attitude windows (aprod1.cu), 3 * xw_axis_stride doubles
-  int att_mode = 1;        // 1 = every start (1 load/axis), 2 = even starts only (half the footprint)
-  int64_t xw_nwin = 0;     // windows per axis
-  int64_t xw_axis_stride = 0;  // doubles between axes in xw (= 4 * xw_nwin)
+  double* att_il = nullptr;   // 3K: interleaved copy of x's attitude block (standalone aprod 1)
+  double* att_acc = nullptr;  // 3K: interleaved attitude accumulator, zero between calls (standalone aprod 2)
   double* ins_copies = nullptr;  // n_copies x I zero-initialised accumulators (only when I*8 exceeds smem)
   int n_copies = 0;
 };
-constexpr size_t ATT_FULL_MAX_BYTES = 40u << 20;  // full expansion only while the table stays L2-resident
 
+constexpr int MAX_TMA_WARPS = 12;                  // warps per CTA of the TMA kernels (register budget 65536 / 384 = 170)
 constexpr size_t SMEM_BUDGET = 227 * 1024 - 512;   // dynamic shared memory we allow one CTA (static: block_sum)
 
 // Launchers (each returns cudaGetLastError()).  Null coefficient pointers mean 1.0 / "no".
+// *_il = the n-vector is LSQR-internal: its attitude block is interleaved, il[3*t + ax] (aprod_device.cuh).
 //   aprod1: y[r] = c1 * (A x)[r] + c0 * y[r]      (c0 = c1 = 1 -> Eq. 2);  *sumsq += sum y[r]^2
 cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* x,
-                          double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
+                          bool x_il, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches);
 //   aprod2: x += A^T (yscale * y)
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
-                          double* x, const double* yscale, const int* done, cudaStream_t st, int64_t* launches);
+                          double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
+                          int64_t* launches);
 cudaError_t launch_validate(const SysView& s, int* flag, cudaStream_t st, int64_t* launches);
-//   fused LSQR step: uh <- A v + c0 uh ; g += A^T uh ; usq += ||uh||^2   (lsqr_fused.cu)
+//   fused LSQR step: uh <- A v + c0 uh ; g += A^T uh ; usq += ||uh||^2   (lsqr_fused.cu; v, g internal layout)
 cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* v,
                               double* uh, double* g, const double* c0, double* usq, int* done, cudaStream_t st,
                               int64_t* launches);
-cudaError_t launch_expand_att(const SysView& s, const SideData& sd, int num_sms, const double* x, const int* done,
-                              cudaStream_t st, int64_t* launches);
+cudaError_t launch_att_to_il(const SysView& s, int num_sms, const double* x_std, double* il, const int* done,
+                             cudaStream_t st, int64_t* launches);
+cudaError_t launch_att_fold(const SysView& s, int num_sms, double* x_std, double* il, cudaStream_t st, int64_t* launches);
+cudaError_t launch_att_from_il(const SysView& s, int num_sms, const double* il, double* dst_std_att, cudaStream_t st,
+                               int64_t* launches);
 cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, const int* done, cudaStream_t st,
                               int64_t* launches);
 cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);

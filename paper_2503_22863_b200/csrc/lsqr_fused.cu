@@ -12,11 +12,12 @@
 
 namespace gsr {
 
-template <int ATT, bool GSMEM, bool ASMEM>
-__global__ void __launch_bounds__(512, 1)
+// v and g are LSQR-internal n-vectors: their attitude blocks are in the interleaved layout (aprod_device.cuh).
+template <bool GSMEM, bool ASMEM>
+__global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
-             const double* __restrict__ xw, int64_t xw_axis_stride, double* __restrict__ uh, double* __restrict__ g,
-             double* ins_copies, int n_copies, const double* __restrict__ c0p, double* usq, int* done) {
+             double* __restrict__ uh, double* __restrict__ g, double* ins_copies, int n_copies,
+             const double* __restrict__ c0p, double* usq, int* done) {
   {
     const int d = *done;
     if (d) {  // LSQR already stopped: no-op (and latch "update pending" 2 -> 1, see k_step_scalars)
@@ -40,9 +41,11 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   if (GSMEM)
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(v + s.oI + i);
   if (ASMEM || GSMEM) __syncthreads();
-  GatherCtx gc{v, xw, xw_axis_stride, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
+  const double* att_il = v + s.oA;
+  GatherCtx gc{v, att_il, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
   ScatterCtx sc{g, g + s.oA, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : g + s.oI,
-                acc_s, s.K};
+                acc_s};
+  const AttLane al(lane);
   const double c0 = *c0p;
   double sq = 0.0, gacc = 0.0;
 
@@ -55,16 +58,19 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    double out = fma(c0, uin, row_dot<ATT, GSMEM>(row, gc));
+    double c[16];
+    att_load_coefs(tile, al, nvalid, c);
+    const double dot = att_dot(al, lane, nvalid, row.i0.y, att_il, c) + row_dot_rest<GSMEM>(row, gc);
+    double out = fma(c0, uin, dot);
     if (valid) {
       uh[r] = out;
       sq = fma(out, out, sq);
     } else {
       out = 0.0;
     }
-    scatter_att(tile, lane, nvalid, out, row.i0.y, sc);
+    ring.release(lane);   // everything this warp needs from the tile is in registers now
+    att_scatter(al, nvalid, out, row.i0.y, sc.gatt_il, c);
     gacc += scatter_row<ASMEM>(row, lane, valid, out, sc);
-    ring.release(lane);
   }
   if (ASMEM) {
     __syncthreads();
@@ -83,36 +89,24 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   }
 }
 
-template <int ATT>
-static cudaError_t launch_fused_t(const SmemPlan& p, const SysView& s, const SideData& sd, int grid, const double* v,
-                                  double* uh, double* g, double* copies, const double* c0, double* usq, int* done,
-                                  cudaStream_t st) {
-  void (*k)(const CUtensorMap, SysView, int, const double*, const double*, int64_t, double*, double*, double*, int,
-            const double*, double*, int*);
-  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<ATT, true, true> : k_lsqr_fused<ATT, true, false>;
-  else k = p.acc_smem ? k_lsqr_fused<ATT, false, true> : k_lsqr_fused<ATT, false, false>;
-  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
-  if (e != cudaSuccess) return e;
-  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, sd.xw, sd.xw_axis_stride, uh, g, copies, sd.n_copies, c0,
-                                          usq, done);
-  return cudaGetLastError();
-}
-
-// expand(v) ; fused pass ; [fold instrumental copies into g]
+// fused pass ; [fold instrumental copies into g]
 cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* v,
                               double* uh, double* g, const double* c0, double* usq, int* done, cudaStream_t st,
                               int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
   const SmemPlan p = plan_smem(s, t, PLAN_FUSED);
-  if (p.bytes > SMEM_BUDGET || p.warps > 16 || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
-  cudaError_t e = launch_expand_att(s, sd, num_sms, v, done, st, launches);
-  if (e != cudaSuccess) return e;
+  if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
   const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
   const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
   double* copies = use_copies ? sd.ins_copies : nullptr;
+  void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, double*, int, const double*, double*, int*);
+  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true> : k_lsqr_fused<true, false>;
+  else k = p.acc_smem ? k_lsqr_fused<false, true> : k_lsqr_fused<false, false>;
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+  if (e != cudaSuccess) return e;
   ++*launches;
-  e = sd.att_mode == ATT_FULL ? launch_fused_t<ATT_FULL>(p, s, sd, grid, v, uh, g, copies, c0, usq, done, st)
-                              : launch_fused_t<ATT_HALF>(p, s, sd, grid, v, uh, g, copies, c0, usq, done, st);
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, copies, sd.n_copies, c0, usq, done);
+  e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (use_copies) return launch_fold_instr(s, sd, g, done, st, launches);
   return cudaSuccess;
