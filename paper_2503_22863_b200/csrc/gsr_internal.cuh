@@ -53,7 +53,10 @@ struct SideData {
   int n_copies = 0;
 };
 
-constexpr int MAX_TMA_WARPS = 12;                  // warps per CTA of the TMA kernels (register budget 65536 / 384 = 170)
+#ifndef GSR_MAX_TMA_WARPS
+#define GSR_MAX_TMA_WARPS 12
+#endif
+constexpr int MAX_TMA_WARPS = GSR_MAX_TMA_WARPS;   // warps per CTA of the TMA kernels (register budget 65536 / 384 = 170)
 constexpr size_t SMEM_BUDGET = 227 * 1024 - 512;   // dynamic shared memory we allow one CTA (static: block_sum)
 
 // Launchers (each returns cudaGetLastError()).  Null coefficient pointers mean 1.0 / "no".
