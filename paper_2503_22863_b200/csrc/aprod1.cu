@@ -36,24 +36,31 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   const double c0 = c0p ? *c0p : 1.0;
   double sq = 0.0;
 
+  double ynext = (gw < ring.n_tiles && gw * TILE_ROWS + lane < s.M) ? y[gw * TILE_ROWS + lane] : 0.0;
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
     const int64_t row0 = t * TILE_ROWS;
     const int64_t r = row0 + lane;
     const bool valid = r < s.M;
-    const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
-    const double yin = valid ? y[r] : 0.0;
-    const char* tile = ring.acquire();
+    const double yin = ynext;
+    {  // prefetch the next tile's y (keeps a DRAM round trip off every tile's critical path)
+      const int64_t rn = r + W * TILE_ROWS;
+      ynext = rn < s.M ? y[rn] : 0.0;
+    }
+    char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    double c[16];
-    att_load_coefs(tile, al, nvalid, c);
-    const double dot = att_dot(al, lane, nvalid, row.i0.y, att_il, c) + row_dot_rest<GSMEM>(row, gc);
-    const double out = fma(c0, yin, dot);
+    int ts[16];
+    att_starts(tile, al, ts);
+    __syncwarp();   // every lane holds its row: the exchange runs may be written
+    att_gather(tile, al, ts, att_il);
+    const double rest = row_dot_rest<GSMEM>(row, gc);
+    __syncwarp();
+    const double out = fma(c0, yin, att_dot_row(tile, lane, row) + rest);
     if (valid) {
       y[r] = out;
       sq = fma(out, out, sq);
     }
-    ring.release(lane);   // after the dependent store: every LDS of this tile has completed
+    ring.release(lane);
   }
   if (sumsq) {
     sq = block_sum(sq);

@@ -30,19 +30,28 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   const double ys = yscale ? *yscale : 1.0;
   double gacc = 0.0;
 
+  double ynext = (gw < ring.n_tiles && gw * TILE_ROWS + lane < s.M) ? y[gw * TILE_ROWS + lane] : 0.0;
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
     const int64_t row0 = t * TILE_ROWS;
     const int64_t r = row0 + lane;
     const bool valid = r < s.M;
-    const double yv = valid ? ys * y[r] : 0.0;
+    const double yv = valid ? ys * ynext : 0.0;
+    {  // prefetch the next tile's y
+      const int64_t rn = r + W * TILE_ROWS;
+      ynext = rn < s.M ? y[rn] : 0.0;
+    }
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
-    const char* tile = ring.acquire();
+    char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    double c[16];
-    att_load_coefs(tile, al, nvalid, c);
-    att_scatter(al, nvalid, yv, row.i0.y, gatt_il, c);
-    gacc += scatter_row<ASMEM>(row, lane, valid, yv, sc);
+    int ts[16];
+    att_starts(tile, al, ts);
+    __syncwarp();   // every lane holds its row: the exchange runs may be written
+    att_products(tile, lane, row, yv);
+    __syncwarp();
+    att_scatter(tile, al, ts, gatt_il);
+    astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x);
+    gacc += scatter_rest<ASMEM>(row, valid, yv, sc);
     ring.release(lane);
   }
   if (ASMEM) {

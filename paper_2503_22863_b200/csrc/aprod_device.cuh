@@ -7,10 +7,14 @@
 // l1tex__m_l1tex2xbar_req_cycles_active and lts__t_tag_requests both ~82 % with the previous
 // design), not DRAM bytes.  So every block of a row is handled in the way that needs the fewest
 // requests:
-//   astro  : lanes of a warp share 1-2 stars -> L1 hits / a segmented warp reduction
+//   astro  : lanes of a warp share 1-2 stars -> L1 hits on the gather side; on the scatter side the
+//            per-star sums of a tile are ONE small matrix product (star indicator x coefficients) done
+//            with eight fp64 DMMA.8x8x4, so no shuffles and 2 reduction instructions per tile
 //   att    : INTERLEAVED attitude layout  il[3*t + ax] = x_att[ax*K + t]: the 12 values a row needs
 //            (3 axes x 4 knots from one start t) are ONE contiguous 96-byte run, fetched / reduced
-//            by 12 consecutive lanes in one instruction (1-2 requests instead of 3-6)
+//            by 12 consecutive lanes in one instruction (1-2 requests instead of 3-6).  The run is
+//            handed between those 12 lanes and the lane that owns the row through the row's own
+//            staged record in shared memory (the "exchange run"), not through shuffles
 //   instr  : shared memory when the slice fits, else L1/L2 gathers and L2 reductions
 #pragma once
 #include "gsr_internal.cuh"
@@ -47,11 +51,19 @@ struct GatherCtx {
   double xg;                // x[oG] (0 when G = 0)
 };
 
-// The lane-per-row part of a staged tile in registers: astro, instrumental, global slots + indices.
+// A staged row: 24 coefficients at a 208-byte stride (tma.cuh).  Once the owning lane holds the row in
+// registers, bytes [XOFF, XOFF+96) of the record (attitude slots 1-11 + instrumental slot 0) are reused
+// as the row's EXCHANGE RUN: 12 doubles in run order p = 3*j + ax (coefficient slot 5 + 4*ax + j),
+// 16-byte aligned so the owner moves it with 6 conflict-free LDS.128 / STS.128 and the cooperative
+// lanes with one LDS.64 / STS.64 per row.  Bytes [OUT_OFF, +8) (zero pad of the TMA box) carry the
+// row's y value for the astrometric matrix product.  Bytes [0, 40) (astro slots) stay intact.
+constexpr int ROW_BYTES = ROW_STRIDE_D * 8;   // 208
+constexpr int XOFF = 48;
+constexpr int OUT_OFF = 192;
+
+// The lane-per-row view of a staged tile in registers: all 24 coefficients + the index record.
 struct RowRegs {
-  double as[5];   // slots 0-4
-  double ai[6];   // slots 17-22
-  double ag;      // slot 23
+  double a[NSLOT];
   int4 i0, i1;    // {star, att_start, instr0, instr1}, {instr2..5}
 };
 
@@ -60,11 +72,13 @@ struct RowRegs {
 // first), which makes the 32-byte-stride pattern bank-conflict free.
 // Tail lanes (row >= M) get zero coefficients (TMA zero fill) and an all-zero index record.
 __device__ __forceinline__ void load_row(const char* tile, int lane, bool valid, RowRegs& r) {
-  const double2* ap = reinterpret_cast<const double2*>(tile + lane * (ROW_STRIDE_D * 8));
-  const double2 c0 = ap[0], c1 = ap[1], c2 = ap[2], c8 = ap[8], c9 = ap[9], c10 = ap[10], c11 = ap[11];
-  r.as[0] = c0.x; r.as[1] = c0.y; r.as[2] = c1.x; r.as[3] = c1.y; r.as[4] = c2.x;
-  r.ai[0] = c8.y; r.ai[1] = c9.x; r.ai[2] = c9.y; r.ai[3] = c10.x; r.ai[4] = c10.y; r.ai[5] = c11.x;
-  r.ag = c11.y;
+  const double2* ap = reinterpret_cast<const double2*>(tile + lane * ROW_BYTES);
+#pragma unroll
+  for (int q = 0; q < NSLOT / 2; q++) {
+    const double2 c = ap[q];
+    r.a[2 * q] = c.x;
+    r.a[2 * q + 1] = c.y;
+  }
   const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
   const int sw = (lane >> 2) & 1;
   const int4 first = ip[sw], second = ip[sw ^ 1];
@@ -73,70 +87,84 @@ __device__ __forceinline__ void load_row(const char* tile, int lane, bool valid,
   if (!valid) { r.i0 = make_int4(0, 0, 0, 0); r.i1 = r.i0; }
 }
 
-// ---- attitude block, cooperative: half-warp h handles row 2*it + h in pass it (16 passes per tile);
-// lane p = lane & 15 < 12 owns position p = 3*j + ax of the row's 96-byte run, i.e. coefficient slot
-// 5 + 4*ax + j.  The LDS.64 of a pass is conflict free (each half-warp reads 12 distinct words-pairs
-// of one row; the two halves are separate wavefronts).
+// ---- attitude block, cooperative side: half-warp h handles row 2*it + h in pass it (16 passes per
+// tile); lane p = lane & 15 < 12 owns position p of the row's 96-byte run.
 struct AttLane {
-  int h, p, slot;
+  int h, p;
   bool act;
-  __device__ __forceinline__ explicit AttLane(int lane) {
-    h = lane >> 4; p = lane & 15; act = p < 12;
-    const int ax = p % 3, j = p / 3;
-    slot = 5 + 4 * ax + j;
-  }
+  __device__ __forceinline__ explicit AttLane(int lane) { h = lane >> 4; p = lane & 15; act = p < 12; }
 };
 
-// c[it] = the lane's attitude coefficient of pass it (0 for idle lanes and rows past the tile's end)
-__device__ __forceinline__ void att_load_coefs(const char* tile, const AttLane& L, int nvalid, double (&c)[16]) {
-  const double* td = reinterpret_cast<const double*>(tile);
+// t[it] = att_start of the row this lane serves in pass it, read from the staged index records (a
+// half-warp broadcast), which nothing overwrites.  Rows past the end of the matrix (ragged last tile)
+// carry zero coefficients (TMA zero fill) and whatever VALID index record the stage held before (the
+// index areas are zeroed at kernel start, TileRing::init): they gather in range and scatter zeros.
+__device__ __forceinline__ void att_starts(const char* tile, const AttLane& L, int (&t)[16]) {
 #pragma unroll
-  for (int it = 0; it < 16; it++) {
-    const int row = 2 * it + L.h;
-    c[it] = (L.act && row < nvalid) ? td[row * ROW_STRIDE_D + L.slot] : 0.0;
+  for (int it = 0; it < 16; it++)
+    t[it] = *reinterpret_cast<const int*>(tile + COEF_TILE_BYTES + (2 * it + L.h) * 32 + 4);
+}
+
+// Gather side: exchange run of row <- x_att(il)[3*t_row .. +12).  16 independent 8-byte loads per lane
+// in flight at once.  Call after every lane has loaded its row (a __syncwarp()).
+__device__ __forceinline__ void att_gather(char* tile, const AttLane& L, const int (&t)[16],
+                                           const double* __restrict__ att_il) {
+  if (L.act) {
+    double v[16];
+#pragma unroll
+    for (int it = 0; it < 16; it++) v[it] = ld_nc_na(att_il + 3 * (int64_t)t[it] + L.p);
+#pragma unroll
+    for (int it = 0; it < 16; it++)
+      *reinterpret_cast<double*>(tile + (2 * it + L.h) * ROW_BYTES + XOFF + 8 * L.p) = v[it];
   }
 }
 
-// Attitude part of (A x)[row of this lane]: sum_{ax,j} a[r][5+4ax+j] * x_att[ax*K + t_r + j].
-// 16 independent 8-byte gathers per lane are in flight at once; the 16 x 16 products of a half-warp
-// are summed by a transposing butterfly (15 shuffle-adds instead of 16 x 4), after which lane p of
-// half h holds the sum of row 2p + h; one more shuffle hands it to the lane that owns the row.
-__device__ __forceinline__ double att_dot(const AttLane& L, int lane, int nvalid, int att_start,
-                                          const double* __restrict__ att_il, const double (&c)[16]) {
-  double v[16];
+// Owner side: sum_{ax,j} a[r][5+4ax+j] * x_att[ax*K + t_r + j] from the row's exchange run.
+__device__ __forceinline__ double att_dot_row(const char* tile, int lane, const RowRegs& r) {
+  const double2* xr = reinterpret_cast<const double2*>(tile + lane * ROW_BYTES + XOFF);
+  double xv[12];
 #pragma unroll
-  for (int it = 0; it < 16; it++) {
-    const int row = 2 * it + L.h;
-    const int t = __shfl_sync(FULL, att_start, row);
-    // unconditional load from a clamped address (a predicated load + select makes ptxas wait for each
-    // load in turn: 16 serialised L2 round trips per tile); idle lanes read element 0 and are masked
-    const bool ok = L.act && row < nvalid;
-    const double xv = ld_nc_na(att_il + (ok ? 3 * (int64_t)t + L.p : 0));
-    v[it] = ok ? c[it] * xv : 0.0;
+  for (int q = 0; q < 6; q++) {
+    const double2 c = xr[q];
+    xv[2 * q] = c.x;
+    xv[2 * q + 1] = c.y;
+  }
+  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
+#pragma unroll
+  for (int j = 0; j < 4; j++) {   // run positions 3j, 3j+1, 3j+2 = axes 0, 1, 2 of knot j
+    acc0 = fma(r.a[5 + j], xv[3 * j], acc0);
+    acc1 = fma(r.a[9 + j], xv[3 * j + 1], acc1);
+    acc2 = fma(r.a[13 + j], xv[3 * j + 2], acc2);
+  }
+  return (acc0 + acc1) + acc2;
+}
+
+// Owner side of the scatter: exchange run of the lane's row <- a[r][slot(p)] * y[r]; pad <- y[r].
+// (The lane only overwrites what it alone reads, so no barrier is needed after att_dot_row.)
+__device__ __forceinline__ void att_products(char* tile, int lane, const RowRegs& r, double yv) {
+  double2* xr = reinterpret_cast<double2*>(tile + lane * ROW_BYTES + XOFF);
+  double pr[12];
+#pragma unroll
+  for (int j = 0; j < 4; j++) {
+    pr[3 * j] = r.a[5 + j] * yv;
+    pr[3 * j + 1] = r.a[9 + j] * yv;
+    pr[3 * j + 2] = r.a[13 + j] * yv;
   }
 #pragma unroll
-  for (int w = 8; w >= 1; w >>= 1) {
-    const bool up = (lane & w) != 0;
-#pragma unroll
-    for (int i = 0; i < w; i++) {
-      const double keep = up ? v[i + w] : v[i];
-      const double send = up ? v[i] : v[i + w];
-      v[i] = keep + __shfl_xor_sync(FULL, send, w);
-    }
-  }
-  return __shfl_sync(FULL, v[0], (lane >> 1) | ((lane & 1) << 4));
+  for (int q = 0; q < 6; q++) xr[q] = make_double2(pr[2 * q], pr[2 * q + 1]);
+  *reinterpret_cast<double*>(tile + lane * ROW_BYTES + OUT_OFF) = yv;
 }
 
 // g_att(il)[3*t_r + p] += a[r][slot(p)] * y[r]  -- PAPER.md:49, Eq. (3), attitude block: per pass one
 // red.global.add.f64 instruction whose 12 active lanes of each half-warp cover one contiguous run.
-__device__ __forceinline__ void att_scatter(const AttLane& L, int nvalid, double yv, int att_start,
-                                            double* __restrict__ gatt_il, const double (&c)[16]) {
+// Call after a __syncwarp() that follows att_products.
+__device__ __forceinline__ void att_scatter(const char* tile, const AttLane& L, const int (&t)[16],
+                                            double* __restrict__ gatt_il) {
+  if (L.act) {
 #pragma unroll
-  for (int it = 0; it < 16; it++) {
-    const int row = 2 * it + L.h;
-    const double yy = __shfl_sync(FULL, yv, row);
-    const int t = __shfl_sync(FULL, att_start, row);
-    if (L.act && row < nvalid) atomicAdd(gatt_il + 3 * (int64_t)t + L.p, c[it] * yy);
+    for (int it = 0; it < 16; it++)
+      atomicAdd(gatt_il + 3 * (int64_t)t[it] + L.p,
+                *reinterpret_cast<const double*>(tile + (2 * it + L.h) * ROW_BYTES + XOFF + 8 * L.p));
   }
 }
 
@@ -152,13 +180,13 @@ __device__ __forceinline__ double row_dot_rest(const RowRegs& r, const GatherCtx
 #pragma unroll
     for (int q = 0; q < 6; q++) g[5 + q] = INSTR_SMEM ? c.xi_s[col[q]] : __ldg(c.xi_g + col[q]);
   }
-  double acc0 = r.ag * c.xg, acc1 = 0.0;
-  acc0 = fma(r.as[0], g[0], acc0); acc1 = fma(r.as[1], g[1], acc1);
-  acc0 = fma(r.as[2], g[2], acc0); acc1 = fma(r.as[3], g[3], acc1);
-  acc0 = fma(r.as[4], g[4], acc0);
-  acc1 = fma(r.ai[0], g[5], acc1); acc0 = fma(r.ai[1], g[6], acc0);
-  acc1 = fma(r.ai[2], g[7], acc1); acc0 = fma(r.ai[3], g[8], acc0);
-  acc1 = fma(r.ai[4], g[9], acc1); acc0 = fma(r.ai[5], g[10], acc0);
+  double acc0 = r.a[23] * c.xg, acc1 = 0.0;
+  acc0 = fma(r.a[0], g[0], acc0); acc1 = fma(r.a[1], g[1], acc1);
+  acc0 = fma(r.a[2], g[2], acc0); acc1 = fma(r.a[3], g[3], acc1);
+  acc0 = fma(r.a[4], g[4], acc0);
+  acc1 = fma(r.a[17], g[5], acc1); acc0 = fma(r.a[18], g[6], acc0);
+  acc1 = fma(r.a[19], g[7], acc1); acc0 = fma(r.a[20], g[8], acc0);
+  acc1 = fma(r.a[21], g[9], acc1); acc0 = fma(r.a[22], g[10], acc0);
   return acc0 + acc1;
 }
 
@@ -170,35 +198,67 @@ struct ScatterCtx {
   double* acc_s;    // shared-memory instrumental accumulator, or nullptr
 };
 
-// Astrometric, instrumental and global slots of the lane's own row, from registers.
-//  astro  (slots 0-4)  : rows are sorted by star, so the lanes of a warp hold runs of equal star; a
-//                        segmented warp scan (shuffles) sums each run, the run head issues 5 adds.
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// x[5*s + k] += sum_{rows r of star s in this tile} a[r][k] * y[r], k < 5   -- Eq. (3), astrometric block.
+// Rows are sorted by star, so a tile covers the consecutive star ids s0 .. s1.  When s1 - s0 < 8 the sums
+// are the 8 x 8 matrix product  C[q][k] = sum_r [star_r == s0 + q] y[r] * a[r][k]  (k < 5), accumulated
+// over the 32 rows by eight fp64 DMMA.8x8x4 whose operands every lane reads straight from the staged
+// tile: A[q][r] = y[r] or 0 (y from the row's pad, star from the index record), B[r][k] = a[r][k]
+// (astro slots, intact).  Lane (q = lane >> 2, i = lane & 3) then owns C[q][2i], C[q][2i+1] and issues
+// at most 2 reductions.  Exact fp64 FMAs (the indicator multiplies by 1 or adds 0).
+// Otherwise (stars with < 5 rows, or unused star ids inside the tile): 5 reductions per row.
+// Requires: att_products(yv) stored (yv = 0 for rows past the end) and a __syncwarp() since.
+__device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nvalid, bool valid, const RowRegs& r,
+                                              double yv, double* __restrict__ x) {
+  const int s0 = __shfl_sync(FULL, r.i0.x, 0), s1 = __shfl_sync(FULL, r.i0.x, nvalid - 1);
+  if (s1 - s0 < 8) {
+    const int q = lane >> 2, i = lane & 3;
+    double c0 = 0.0, c1 = 0.0, d0 = 0.0, d1 = 0.0;   // two independent accumulation chains
+#pragma unroll
+    for (int j = 0; j < 8; j++) {
+      const int row = 4 * j + i;
+      const int st = *reinterpret_cast<const int*>(tile + COEF_TILE_BYTES + row * 32);
+      const double y = *reinterpret_cast<const double*>(tile + row * ROW_BYTES + OUT_OFF);
+      const double b = *reinterpret_cast<const double*>(tile + row * ROW_BYTES + 8 * (q < 5 ? q : 0));
+      if (j & 1) dmma884(d0, d1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
+      else dmma884(c0, c1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
+    }
+    c0 += d0;
+    c1 += d1;
+    if (q <= s1 - s0 && i < 3) {
+      double* xa = x + 5 * (int64_t)(s0 + q) + 2 * i;
+      atomicAdd(xa, c0);
+      if (i < 2) atomicAdd(xa + 1, c1);
+    }
+  } else if (valid) {
+    double* xa = x + 5 * (int64_t)r.i0.x;
+#pragma unroll
+    for (int k = 0; k < 5; k++) atomicAdd(xa + k, r.a[k] * yv);
+  }
+}
+
+// Instrumental and global slots of the lane's own row, from registers.
 //  instr  (slots 17-22): block-privatised accumulators in shared memory when the slice fits (flushed
 //                        once per CTA), else reductions at L2.
 //  global (slot 23)    : returned as the lane's contribution, reduced once per CTA by the caller.
+//  (Shared memory has no native fp64 add: atomicAdd is an LDS / DADD / ATOMS.CAST.SPIN loop.  Running the
+//  six chains of a row side by side with plain atomicCAS was measured SLOWER: aprod 2 at C2 0.72 vs 0.52 ms.)
 template <bool INSTR_SMEM>
-__device__ __forceinline__ double scatter_row(const RowRegs& r, int lane, bool valid, double yv, const ScatterCtx& c) {
-  const int star = valid ? r.i0.x : (-1 - lane);
-  double p0 = r.as[0] * yv, p1 = r.as[1] * yv, p2 = r.as[2] * yv, p3 = r.as[3] * yv, p4 = r.as[4] * yv;
-#pragma unroll
-  for (int off = 1; off < 32; off <<= 1) {
-    const int so = __shfl_down_sync(FULL, star, off);
-    const double q0 = __shfl_down_sync(FULL, p0, off), q1 = __shfl_down_sync(FULL, p1, off),
-                 q2 = __shfl_down_sync(FULL, p2, off), q3 = __shfl_down_sync(FULL, p3, off),
-                 q4 = __shfl_down_sync(FULL, p4, off);
-    if (lane + off < 32 && so == star) { p0 += q0; p1 += q1; p2 += q2; p3 += q3; p4 += q4; }
-  }
-  const int sprev = __shfl_up_sync(FULL, star, 1);
-  if (valid && (lane == 0 || sprev != star)) {   // head of a run of equal star
-    double* xa = c.x + 5 * (int64_t)star;
-    atomicAdd(xa, p0); atomicAdd(xa + 1, p1); atomicAdd(xa + 2, p2); atomicAdd(xa + 3, p3); atomicAdd(xa + 4, p4);
-  }
+__device__ __forceinline__ double scatter_rest(const RowRegs& r, bool valid, double yv, const ScatterCtx& c) {
   double gl = 0.0;
   if (valid) {
+    const int col[6] = {r.i0.z, r.i0.w, r.i1.x, r.i1.y, r.i1.z, r.i1.w};
+    double inc[6];
+#pragma unroll
+    for (int q = 0; q < 6; q++) inc[q] = r.a[17 + q] * yv;
     double* t = INSTR_SMEM ? c.acc_s : c.xins;
-    atomicAdd(t + r.i0.z, r.ai[0] * yv); atomicAdd(t + r.i0.w, r.ai[1] * yv); atomicAdd(t + r.i1.x, r.ai[2] * yv);
-    atomicAdd(t + r.i1.y, r.ai[3] * yv); atomicAdd(t + r.i1.z, r.ai[4] * yv); atomicAdd(t + r.i1.w, r.ai[5] * yv);
-    gl = r.ag * yv;
+#pragma unroll
+    for (int q = 0; q < 6; q++) atomicAdd(t + col[q], inc[q]);
+    gl = r.a[23] * yv;
   }
   return gl;
 }

@@ -49,28 +49,39 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   const double c0 = *c0p;
   double sq = 0.0, gacc = 0.0;
 
+  double unext = (gw < ring.n_tiles && gw * TILE_ROWS + lane < s.M) ? uh[gw * TILE_ROWS + lane] : 0.0;
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
     const int64_t row0 = t * TILE_ROWS;
     const int64_t r = row0 + lane;
     const bool valid = r < s.M;
-    const double uin = valid ? uh[r] : 0.0;
+    const double uin = unext;
+    {  // prefetch the next tile's u: a DRAM round trip that would otherwise sit on every tile's critical path
+      const int64_t rn = r + W * TILE_ROWS;
+      unext = rn < s.M ? uh[rn] : 0.0;
+    }
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
-    const char* tile = ring.acquire();
+    char* tile = ring.acquire();
     RowRegs row;
     load_row(tile, lane, valid, row);
-    double c[16];
-    att_load_coefs(tile, al, nvalid, c);
-    const double dot = att_dot(al, lane, nvalid, row.i0.y, att_il, c) + row_dot_rest<GSMEM>(row, gc);
-    double out = fma(c0, uin, dot);
+    int ts[16];
+    att_starts(tile, al, ts);
+    __syncwarp();   // every lane holds its row: the exchange runs may be written
+    att_gather(tile, al, ts, att_il);
+    const double rest = row_dot_rest<GSMEM>(row, gc);
+    __syncwarp();
+    double out = fma(c0, uin, att_dot_row(tile, lane, row) + rest);
     if (valid) {
       uh[r] = out;
       sq = fma(out, out, sq);
     } else {
       out = 0.0;
     }
-    ring.release(lane);   // everything this warp needs from the tile is in registers now
-    att_scatter(al, nvalid, out, row.i0.y, sc.gatt_il, c);
-    gacc += scatter_row<ASMEM>(row, lane, valid, out, sc);
+    att_products(tile, lane, row, out);
+    __syncwarp();
+    att_scatter(tile, al, ts, sc.gatt_il);
+    astro_scatter(tile, lane, nvalid, valid, row, out, sc.x);
+    gacc += scatter_rest<ASMEM>(row, valid, out, sc);
+    ring.release(lane);
   }
   if (ASMEM) {
     __syncthreads();

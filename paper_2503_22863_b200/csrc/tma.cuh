@@ -44,6 +44,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "DONE_%=:\n"
       "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
   uint64_t p;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
@@ -95,12 +96,18 @@ struct TileRing {
     n_tiles = (M_ + TILE_ROWS - 1) / TILE_ROWS;
     stride = stride_; next_issue = first_tile; stage = 0; phase = 0;
     policy = l2_policy_evict_first();
+    // index areas start as all-zero records, so that the rows of a ragged last tile that the copy does
+    // not cover always hold in-range indices (zeros or an earlier tile's records)
+    for (int s = 0; s < nstages; s++)
+      reinterpret_cast<int4*>(base + s * STAGE_BYTES + COEF_TILE_BYTES)[lane] = make_int4(0, 0, 0, 0),
+      reinterpret_cast<int4*>(base + s * STAGE_BYTES + COEF_TILE_BYTES)[32 + lane] = make_int4(0, 0, 0, 0);
     if (lane == 0) {
       for (int s = 0; s < nstages; s++) mbar_init(bars + s, 1);
       mbar_fence_init();
     }
     __syncwarp();
     if (lane == 0) {
+      fence_proxy_async();
       for (int s = 0; s < nstages; s++) {
         if (next_issue < n_tiles) issue(s, next_issue);
         next_issue += stride;
@@ -110,14 +117,18 @@ struct TileRing {
   }
 
   // wait until the current tile has landed; returns its shared-memory address
-  __device__ __forceinline__ const char* acquire() {
+  __device__ __forceinline__ char* acquire() {
     mbar_wait(bars + stage, phase);
     return base + stage * STAGE_BYTES;
   }
-  // the warp is done reading the current tile: refill its stage with the next tile of the sequence
+  // the warp is done with the current tile (it may have written into it: exchange runs, aprod_device.cuh):
+  // order those generic-proxy accesses before the async-proxy refill, then request the next tile
   __device__ __forceinline__ void release(int lane) {
     __syncwarp();
-    if (lane == 0 && next_issue < n_tiles) issue(stage, next_issue);
+    if (lane == 0 && next_issue < n_tiles) {
+      fence_proxy_async();
+      issue(stage, next_issue);
+    }
     next_issue += stride;
     if (++stage == nstages) { stage = 0; phase ^= 1; }
   }

@@ -99,9 +99,11 @@ def test_aprod_c1():
         check_aprod2(C1, a, idx, s, 5, x_in=np.zeros(8061))
 
 
-@pytest.mark.parametrize("n_stars,obs", [(1, 1), (1, 31), (1, 33), (3, 11), (7, 37), (5, 129), (2, 1000), (64, 64)])
+@pytest.mark.parametrize("n_stars,obs", [(1, 1), (1, 31), (1, 33), (3, 11), (7, 37), (5, 129), (2, 1000), (64, 64),
+                                         (300, 1), (150, 3), (41, 5)])
 def test_aprod_ragged_sizes(n_stars, obs):
-    """Row counts around the 32-row tile: single row, ragged tails, several tiles, one long star."""
+    """Row counts around the 32-row tile: single row, ragged tails, several tiles, one long star; stars
+    with 1-5 rows (a tile then spans 8 or more star ids: the non-matrix-product astrometric path)."""
     shape = tiny_shape(n_stars=n_stars, obs=obs, n_knots=50, n_instr=17, seed=100 + obs)
     a, idx = host.make_rows(shape)
     with make_gpu_system(shape, a, idx) as s:
