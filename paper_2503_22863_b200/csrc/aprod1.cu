@@ -134,8 +134,8 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   if (ring > SMEM_BUDGET) { p.bytes = ring; return p; }   // caller rejects (cudaErrorInvalidValue)
   size_t left = SMEM_BUDGET - ring;
   // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1 gathers per row
-  if ((what & PLAN_APROD2) && table <= left) { p.acc_smem = true; left -= table; }
-  if ((what & PLAN_APROD1) && table <= left) { p.gather_smem = true; left -= table; }
+  if ((what & PLAN_APROD2) && t.acc_smem && table <= left) { p.acc_smem = true; left -= table; }
+  if ((what & PLAN_APROD1) && t.gather_smem && table <= left) { p.gather_smem = true; left -= table; }
   p.bytes = SMEM_BUDGET - left;
   return p;
 }
