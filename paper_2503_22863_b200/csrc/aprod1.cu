@@ -124,18 +124,28 @@ cudaError_t launch_att_from_il(const SysView& s, int num_sms, const double* il, 
 // ---- shared-memory plan of the TMA kernels --------------------------------------------------------
 static size_t ring_bytes(int w, int st) { return (size_t)w * st * STAGE_BYTES + (size_t)(w * st + 2) * 8 + 128; }
 
+// Warps per CTA trade latency hiding against room for the instrumental tables.  Measured (B200, fused
+// pass / aprod 1 / aprod 2): C3 (I = 6,000) 12 warps without tables 4.89 / 2.39 / 4.25 ms, 8 warps with the
+// tables 4.19 / 1.90 / 2.70 ms; C5 (I = 12,000, only one table fits at 8 warps) 14.6 / 8.68 / 12.0 ms with
+// 12 warps, 17.6 / 6.82 / 8.48 ms with 8.  So: the most warps (12 down to 8) at which EVERY table the kernel
+// wants fits; if there is no such count, 12 warps and whatever still fits.
 SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   SmemPlan p;
-  p.warps = t.warps > 0 ? t.warps : 12;
   p.stages = t.stages > 0 ? t.stages : 2;
   p.gather_smem = p.acc_smem = false;
   const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
+  const bool want_acc = (what & PLAN_APROD2) && t.acc_smem, want_gather = (what & PLAN_APROD1) && t.gather_smem;
+  const size_t want = (want_acc ? table : 0) + (want_gather ? table : 0);
+  p.warps = t.warps > 0 ? t.warps : 12;
+  if (t.warps <= 0 && want > 0)
+    for (int w = 12; w >= 8; w--)
+      if (ring_bytes(w, p.stages) + want <= SMEM_BUDGET) { p.warps = w; break; }
   size_t ring = ring_bytes(p.warps, p.stages);
   if (ring > SMEM_BUDGET) { p.bytes = ring; return p; }   // caller rejects (cudaErrorInvalidValue)
   size_t left = SMEM_BUDGET - ring;
-  // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1 gathers per row
-  if ((what & PLAN_APROD2) && t.acc_smem && table <= left) { p.acc_smem = true; left -= table; }
-  if ((what & PLAN_APROD1) && t.gather_smem && table <= left) { p.gather_smem = true; left -= table; }
+  // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1/L2 gathers per row
+  if (want_acc && table <= left) { p.acc_smem = true; left -= table; }
+  if (want_gather && table <= left) { p.gather_smem = true; left -= table; }
   p.bytes = SMEM_BUDGET - left;
   return p;
 }

@@ -102,10 +102,10 @@ static int build_att_buffers(gsr_system* s) {
 }
 
 // Replicated instrumental accumulators in global memory (L2-resident): one per CTA while that stays
-// under 16 MB, at least 8 (60,000 addresses hit by 3e9 reductions are contention-bound otherwise).
+// under 4 MB, at least 8 (60,000 addresses hit by 3e9 reductions are contention-bound otherwise).
 static int build_instr_copies(gsr_system* s) {
   const SysView& v = s->v;
-  int64_t copies = (int64_t)(16u << 20) / (v.I * 8);
+  int64_t copies = (int64_t)(4u << 20) / (v.I * 8);
   if (copies > s->num_sms) copies = s->num_sms;
   if (copies < 8) copies = 8;
   cudaError_t e = cudaMalloc(&s->side.ins_copies, (size_t)copies * v.I * sizeof(double));
