@@ -133,13 +133,18 @@ def measured_peak():
 
 
 def ncu_traffic(kernel, m):
-    """dram bytes per launch from the committed ncu --set full summary, scaled by rows; else None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per launch from the committed ncu --set full summary (profiles/r01_traffic.csv:
+    bytes per row of one captured launch), scaled by the rows of this workload; else None."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
     try:
-        t = json.load(open(p))
-        return float(t[kernel]["dram_bytes_per_row"]) * m
+        with open(p) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel:
+                    return float(row["dram_bytes_per_row"]) * m
     except Exception:
-        return None
+        pass
+    return None
 
 
 def pick_workload(name, free_bytes):
