@@ -148,7 +148,17 @@ int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int
  * gsr_profile_get  : after a synchronise, mean duration in ms and launch count since the last
  *                    call, per kernel class: which = 1 aprod1, 2 aprod2, 3 the fused LSQR pass
  *                    (aprod 1 + aprod 2 of one iteration in one sweep over A) (host out-pointers).
- * gsr_set_option   : tuning knobs; unknown names -> GSR_EINVAL.          */
+ * gsr_set_option   : tuning knobs (measured in profiles/r01_summary.md section 3);
+ *                    unknown names -> GSR_EINVAL.  Names (value 0 = default of the planner unless stated):
+ *                      warps, stages     warps per CTA (<= 12) and TMA ring depth per warp of the tile kernels
+ *                      ctas_per_sm       CTAs per SM (default 1)
+ *                      acc_smem          1 (default) privatise the instrumental accumulators in shared memory
+ *                                        when they fit, 0 always reduce into the L2-resident copies
+ *                      gather_smem       1 (default) stage the instrumental slice of x in shared memory when it fits
+ *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x
+ *                      fused             1 (default) one pass over A per LSQR iteration, 0 aprod 1 then aprod 2
+ *                      aprod1_variant, aprod2_variant   1 (default) TMA tiles, 0 one thread per row (cross-check)
+ *                      check_every       LSQR iterations between host polls of the stop flag (default 16)      */
 int gsr_launch_count(const gsr_system *sys, int64_t *n_launches);
 int gsr_profile(gsr_system *sys, int enable);
 int gsr_profile_get(gsr_system *sys, int which, double *mean_ms, int64_t *count);
