@@ -26,7 +26,7 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
-  ring.init(ring_mem, bars + warp * nstages, &map, s.idx, s.M, gw, W, lane, nstages);
+  ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
   if (GSMEM) {
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(x + s.oI + i);
     __syncthreads();
@@ -46,7 +46,7 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
       const int64_t rn = r + W * TILE_ROWS;
       ynext = rn < s.M ? y[rn] : 0.0;
     }
-    char* tile = ring.acquire();
+    char* tile = ring.acquire(t, lane);
     RowRegs row;
     load_row(tile, lane, valid, row);
     int ts[16];

@@ -1,6 +1,6 @@
 // Per-tile device routines shared by the aprod1, aprod2 and fused LSQR kernels.
-// A tile is 32 rows staged in shared memory by TMA (tma.cuh): coefficients with a 208-byte row
-// stride, then the 32 index records.
+// A tile is 32 rows staged in shared memory by TMA (tma.cuh): coefficients as 16 row pairs with a
+// 400-byte pair stride, then the 32 index records.
 //
 // What bounds these kernels on B200 is the number of L2 requests per row (each SM can send one
 // request per cycle to the crossbar, each of the 184 L2 slices looks up one tag per cycle; ncu:
@@ -51,15 +51,13 @@ struct GatherCtx {
   double xg;                // x[oG] (0 when G = 0)
 };
 
-// A staged row: 24 coefficients at a 208-byte stride (tma.cuh).  Once the owning lane holds the row in
-// registers, bytes [XOFF, XOFF+96) of the record (attitude slots 1-11 + instrumental slot 0) are reused
-// as the row's EXCHANGE RUN: 12 doubles in run order p = 3*j + ax (coefficient slot 5 + 4*ax + j),
+// A staged row: 24 coefficients at row_off(r) of the tile (tma.cuh).  Once the owning lane holds the row
+// in registers, bytes [XOFF, XOFF+96) of the record (attitude slots 1-11 + instrumental slot 0) are
+// reused as the row's EXCHANGE RUN: 12 doubles in run order p = 3*j + ax (coefficient slot 5 + 4*ax + j),
 // 16-byte aligned so the owner moves it with 6 conflict-free LDS.128 / STS.128 and the cooperative
-// lanes with one LDS.64 / STS.64 per row.  Bytes [OUT_OFF, +8) (zero pad of the TMA box) carry the
+// lanes with one LDS.64 / STS.64 per row.  The 8 bytes at pad_off(r) (zero pad of the TMA box) carry the
 // row's y value for the astrometric matrix product.  Bytes [0, 40) (astro slots) stay intact.
-constexpr int ROW_BYTES = ROW_STRIDE_D * 8;   // 208
 constexpr int XOFF = 48;
-constexpr int OUT_OFF = 192;
 
 // The lane-per-row view of a staged tile in registers: all 24 coefficients + the index record.
 struct RowRegs {
@@ -67,12 +65,12 @@ struct RowRegs {
   int4 i0, i1;    // {star, att_start, instr0, instr1}, {instr2..5}
 };
 
-// Lane l reads row l of the tile: conflict-free LDS.128 (208-byte stride), and the 32-byte index
+// Lane l reads row l of the tile: conflict-free LDS.128 (row_off, tma.cuh), and the 32-byte index
 // record as two LDS.128 issued in swizzled order (lanes 4-7, 12-15, ... read the second half
 // first), which makes the 32-byte-stride pattern bank-conflict free.
 // Tail lanes (row >= M) get zero coefficients (TMA zero fill) and an all-zero index record.
 __device__ __forceinline__ void load_row(const char* tile, int lane, bool valid, RowRegs& r) {
-  const double2* ap = reinterpret_cast<const double2*>(tile + lane * ROW_BYTES);
+  const double2* ap = reinterpret_cast<const double2*>(tile + row_off(lane));
 #pragma unroll
   for (int q = 0; q < NSLOT / 2; q++) {
     const double2 c = ap[q];
@@ -115,13 +113,13 @@ __device__ __forceinline__ void att_gather(char* tile, const AttLane& L, const i
     for (int it = 0; it < 16; it++) v[it] = ld_nc_na(att_il + 3 * (int64_t)t[it] + L.p);
 #pragma unroll
     for (int it = 0; it < 16; it++)
-      *reinterpret_cast<double*>(tile + (2 * it + L.h) * ROW_BYTES + XOFF + 8 * L.p) = v[it];
+      *reinterpret_cast<double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p) = v[it];
   }
 }
 
 // Owner side: sum_{ax,j} a[r][5+4ax+j] * x_att[ax*K + t_r + j] from the row's exchange run.
 __device__ __forceinline__ double att_dot_row(const char* tile, int lane, const RowRegs& r) {
-  const double2* xr = reinterpret_cast<const double2*>(tile + lane * ROW_BYTES + XOFF);
+  const double2* xr = reinterpret_cast<const double2*>(tile + row_off(lane) + XOFF);
   double xv[12];
 #pragma unroll
   for (int q = 0; q < 6; q++) {
@@ -142,7 +140,7 @@ __device__ __forceinline__ double att_dot_row(const char* tile, int lane, const 
 // Owner side of the scatter: exchange run of the lane's row <- a[r][slot(p)] * y[r]; pad <- y[r].
 // (The lane only overwrites what it alone reads, so no barrier is needed after att_dot_row.)
 __device__ __forceinline__ void att_products(char* tile, int lane, const RowRegs& r, double yv) {
-  double2* xr = reinterpret_cast<double2*>(tile + lane * ROW_BYTES + XOFF);
+  double2* xr = reinterpret_cast<double2*>(tile + row_off(lane) + XOFF);
   double pr[12];
 #pragma unroll
   for (int j = 0; j < 4; j++) {
@@ -152,7 +150,7 @@ __device__ __forceinline__ void att_products(char* tile, int lane, const RowRegs
   }
 #pragma unroll
   for (int q = 0; q < 6; q++) xr[q] = make_double2(pr[2 * q], pr[2 * q + 1]);
-  *reinterpret_cast<double*>(tile + lane * ROW_BYTES + OUT_OFF) = yv;
+  *reinterpret_cast<double*>(tile + pad_off(lane)) = yv;
 }
 
 // g_att(il)[3*t_r + p] += a[r][slot(p)] * y[r]  -- PAPER.md:49, Eq. (3), attitude block: per pass one
@@ -164,7 +162,7 @@ __device__ __forceinline__ void att_scatter(const char* tile, const AttLane& L, 
 #pragma unroll
     for (int it = 0; it < 16; it++)
       atomicAdd(gatt_il + 3 * (int64_t)t[it] + L.p,
-                *reinterpret_cast<const double*>(tile + (2 * it + L.h) * ROW_BYTES + XOFF + 8 * L.p));
+                *reinterpret_cast<const double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p));
   }
 }
 
@@ -222,8 +220,8 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
     for (int j = 0; j < 8; j++) {
       const int row = 4 * j + i;
       const int st = *reinterpret_cast<const int*>(tile + COEF_TILE_BYTES + row * 32);
-      const double y = *reinterpret_cast<const double*>(tile + row * ROW_BYTES + OUT_OFF);
-      const double b = *reinterpret_cast<const double*>(tile + row * ROW_BYTES + 8 * (q < 5 ? q : 0));
+      const double y = *reinterpret_cast<const double*>(tile + pad_off(row));
+      const double b = *reinterpret_cast<const double*>(tile + row_off(row) + 8 * (q < 5 ? q : 0));
       if (j & 1) dmma884(d0, d1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
       else dmma884(c0, c1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
     }

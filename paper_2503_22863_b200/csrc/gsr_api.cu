@@ -74,9 +74,10 @@ static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
     return cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
-  const cuuint64_t dims[2] = {(cuuint64_t)NSLOT, (cuuint64_t)(M > 0 ? M : 1)};
-  const cuuint64_t strides[1] = {(cuuint64_t)NSLOT * sizeof(double)};       // 192-byte rows
-  const cuuint32_t box[2] = {26u, 32u};                                      // 24 + 2 zero-filled pad columns
+  // pair view (tma.cuh): one tensor row = two matrix rows = 384 bytes; the last row of an odd M is not covered
+  const cuuint64_t dims[2] = {(cuuint64_t)(2 * NSLOT), (cuuint64_t)(M >= 2 ? M / 2 : 1)};
+  const cuuint64_t strides[1] = {(cuuint64_t)(2 * NSLOT) * sizeof(double)};
+  const cuuint32_t box[2] = {50u, 16u};                                      // 48 + 2 zero-filled pad columns
   const cuuint32_t estr[2] = {1u, 1u};
   CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(values),
                                                    dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,

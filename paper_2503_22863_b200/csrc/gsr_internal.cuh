@@ -48,7 +48,7 @@ struct Tuning {
 
 // Side structures owned by the library (built in gsr_create).
 struct SideData {
-  CUtensorMap map;         // 24 x M fp64 tensor, box 26 x 32 (tma.cuh)
+  CUtensorMap map;         // 48 x floor(M/2) fp64 tensor (row pairs), box 50 x 16 (tma.cuh)
   double* att_il = nullptr;   // 3K: interleaved copy of x's attitude block (standalone aprod 1)
   double* att_acc = nullptr;  // 3K: interleaved attitude accumulator, zero between calls (standalone aprod 2)
   double* ins_copies = nullptr;  // n_copies x I zero-initialised accumulators (only when I*8 exceeds smem)

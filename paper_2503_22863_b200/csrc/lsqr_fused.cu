@@ -35,7 +35,7 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
-  ring.init(ring_mem, bars + warp * nstages, &map, s.idx, s.M, gw, W, lane, nstages);
+  ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
   if (ASMEM)
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
   if (GSMEM)
@@ -60,7 +60,7 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
       unext = rn < s.M ? uh[rn] : 0.0;
     }
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
-    char* tile = ring.acquire();
+    char* tile = ring.acquire(t, lane);
     RowRegs row;
     load_row(tile, lane, valid, row);
     int ts[16];

@@ -2,12 +2,15 @@
 // aprod kernels.
 //
 // Row tile = 32 consecutive rows.  Its 24-coefficient records (32 x 192 B, contiguous in HBM) are
-// fetched by ONE tensor-map TMA load whose box is 26 x 32 doubles on a tensor of extent 24 x M:
-// columns 24,25 are out of bounds and zero-filled, so every row lands in shared memory with a
-// 208-byte stride.  208 = 13 * 16, an odd number of 16-byte chunks, which makes the lane-per-row
-// LDS.128 pattern (lane l reads chunk c of row l) bank-conflict free; a dense 192-byte stride
-// would be a 4-way conflict.  Rows past M are zero-filled the same way (ragged tail).
-// The 32 index records (32 x 32 B) follow with one 1-D bulk copy.
+// fetched by ONE tensor-map TMA load.  The tensor view pairs the rows: extent 48 x floor(M/2) doubles,
+// i.e. one tensor row = two matrix rows = 384 B = three whole 128-byte lines, so the stream costs 1.5 L2
+// requests per matrix row (a 24 x M view with 192-byte tensor rows costs 2-3).  The box is 50 x 16:
+// columns 48,49 are out of bounds and zero-filled, so every PAIR lands in shared memory with a 400-byte
+// stride and the rows of a pair 192 B apart.  400 = 25 * 16 and 192 = 12 * 16 make the lane-per-row
+// LDS.128 pattern (lane l reads chunk c of row l) bank-conflict free: the 16-byte chunk positions
+// (25 * (l >> 1) + 12 * (l & 1) + c) mod 8 take each value exactly four times over a warp.  Pairs past
+// floor(M/2) are zero-filled the same way (ragged tail); the last row of an odd M is copied by the warp
+// itself (TileRing::acquire).  The 32 index records (32 x 32 B) follow with one 1-D bulk copy.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -16,10 +19,14 @@
 namespace gsr {
 
 constexpr int TILE_ROWS = 32;
-constexpr int ROW_STRIDE_D = 26;                               // doubles per staged row (24 + 2 zero pad)
-constexpr int COEF_TILE_BYTES = TILE_ROWS * ROW_STRIDE_D * 8;  // 6656
+constexpr int PAIR_BYTES = 400;                                // two 192-byte rows + 16 bytes of zero pad
+constexpr int COEF_TILE_BYTES = (TILE_ROWS / 2) * PAIR_BYTES;  // 6400
 constexpr int IDX_TILE_BYTES = TILE_ROWS * 32;                 // 1024
-constexpr int STAGE_BYTES = COEF_TILE_BYTES + IDX_TILE_BYTES;  // 7680 (multiple of 128)
+constexpr int STAGE_BYTES = COEF_TILE_BYTES + IDX_TILE_BYTES;  // 7424 (multiple of 128)
+
+// byte offset of row r (0..31) of a staged tile, and of the 8-byte pad slot that belongs to it
+__host__ __device__ constexpr int row_off(int r) { return (r >> 1) * PAIR_BYTES + (r & 1) * 192; }
+__host__ __device__ constexpr int pad_off(int r) { return (r >> 1) * PAIR_BYTES + 384 + (r & 1) * 8; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -72,6 +79,7 @@ struct TileRing {
   char* base;       // this warp's STAGES * STAGE_BYTES of shared memory (128-byte aligned)
   uint64_t* bars;   // this warp's STAGES mbarriers
   const CUtensorMap* map;
+  const double* vals;
   const int32_t* idx;
   int64_t M, n_tiles, stride;   // stride = number of warps sharing the tile sequence
   int64_t next_issue;           // next tile this warp will request
@@ -85,14 +93,16 @@ struct TileRing {
     const int64_t left = M - row0;
     const uint32_t idx_bytes = static_cast<uint32_t>((left < TILE_ROWS ? left : TILE_ROWS) * 32);
     char* dst = base + s * STAGE_BYTES;
-    mbar_expect_tx(bars + s, COEF_TILE_BYTES + idx_bytes);
-    tma_load_2d(dst, map, 0, static_cast<int>(row0), bars + s, policy);
+    const bool pairs = row0 + 1 < M;   // the tile holds at least one whole pair (else: a single last row)
+    mbar_expect_tx(bars + s, (pairs ? COEF_TILE_BYTES : 0) + idx_bytes);
+    if (pairs) tma_load_2d(dst, map, 0, static_cast<int>(row0 >> 1), bars + s, policy);
     bulk_load_1d(dst + COEF_TILE_BYTES, idx + row0 * 8, idx_bytes, bars + s, policy);
   }
 
-  __device__ __forceinline__ void init(char* smem_base, uint64_t* bar_base, const CUtensorMap* m, const int32_t* idx_,
-                                       int64_t M_, int64_t first_tile, int64_t stride_, int lane, int nstages_) {
-    base = smem_base; bars = bar_base; map = m; idx = idx_; M = M_; nstages = nstages_;
+  __device__ __forceinline__ void init(char* smem_base, uint64_t* bar_base, const CUtensorMap* m, const double* vals_,
+                                       const int32_t* idx_, int64_t M_, int64_t first_tile, int64_t stride_, int lane,
+                                       int nstages_) {
+    base = smem_base; bars = bar_base; map = m; vals = vals_; idx = idx_; M = M_; nstages = nstages_;
     n_tiles = (M_ + TILE_ROWS - 1) / TILE_ROWS;
     stride = stride_; next_issue = first_tile; stage = 0; phase = 0;
     policy = l2_policy_evict_first();
@@ -116,10 +126,21 @@ struct TileRing {
     next_issue = __shfl_sync(0xffffffffu, next_issue, 0);
   }
 
-  // wait until the current tile has landed; returns its shared-memory address
-  __device__ __forceinline__ char* acquire() {
+  // wait until tile t (the current one) has landed; returns its shared-memory address
+  __device__ __forceinline__ char* acquire(int64_t t, int lane) {
     mbar_wait(bars + stage, phase);
-    return base + stage * STAGE_BYTES;
+    char* tile = base + stage * STAGE_BYTES;
+    if ((M & 1) && t == n_tiles - 1) {
+      // odd M: the last row has no partner, so the pair view does not cover it.  The warp copies it
+      // (and clears the coefficient area first when the tile is that single row and no TMA load ran).
+      const int last = static_cast<int>(M - 1 - t * TILE_ROWS);
+      if (last == 0)
+        for (int i = lane; i < COEF_TILE_BYTES / 16; i += 32) reinterpret_cast<int4*>(tile)[i] = make_int4(0, 0, 0, 0);
+      __syncwarp();
+      if (lane < 24) reinterpret_cast<double*>(tile + row_off(last))[lane] = vals[(M - 1) * 24 + lane];
+      __syncwarp();
+    }
+    return tile;
   }
   // the warp is done with the current tile (it may have written into it: exchange runs, aprod_device.cuh):
   // order those generic-proxy accesses before the async-proxy refill, then request the next tile
