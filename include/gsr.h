@@ -154,6 +154,8 @@ int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int
  *                      ctas_per_sm       CTAs per SM (default 1)
  *                      acc_smem          1 (default) privatise the instrumental accumulators in shared memory
  *                                        when they fit, 0 always reduce into the L2-resident copies
+ *                      die_local         1 (default) L2-resident instrumental accumulators: every CTA reduces into a copy whose
+ *                                        4 KB chunks are homed on the L2 of its own die (probed at gsr_create), 0 control
  *                      gather_smem       1 (default) stage the instrumental slice of x in shared memory when it fits
  *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x
  *                      fused             1 (default) one pass over A per LSQR iteration, 0 aprod 1 then aprod 2
@@ -163,6 +165,10 @@ int gsr_launch_count(const gsr_system *sys, int64_t *n_launches);
 int gsr_profile(gsr_system *sys, int enable);
 int gsr_profile_get(gsr_system *sys, int which, double *mean_ms, int64_t *count);
 int gsr_set_option(gsr_system *sys, const char *name, int64_t value);
+/* gsr_instr_acc_info : what gsr_create found when it probed the L2 home die of the instrumental accumulator
+ *                      chunks.  info (host, 5 x int32) = {two dies seen (0/1), copies per
+ *                      die, 4 KB chunks per copy, SMs found on die 0, SMs found on die 1}.                        */
+int gsr_instr_acc_info(const gsr_system *sys, int32_t *info);
 const char *gsr_strerror(int code);
 const char *gsr_last_cuda_error(void); /* text of the last CUDA failure in this thread, or "" */
 const char *gsr_version(void);

@@ -71,6 +71,7 @@ SYMBOLS = {
     "gsr_profile": (ct.c_int, [_vp, ct.c_int]),
     "gsr_profile_get": (ct.c_int, [_vp, ct.c_int, ct.POINTER(ct.c_double), ct.POINTER(ct.c_int64)]),
     "gsr_set_option": (ct.c_int, [_vp, ct.c_char_p, ct.c_int64]),
+    "gsr_instr_acc_info": (ct.c_int, [_vp, ct.POINTER(ct.c_int32)]),
     "gsr_strerror": (ct.c_char_p, [ct.c_int]),
     "gsr_last_cuda_error": (ct.c_char_p, []),
     "gsr_version": (ct.c_char_p, []),
@@ -224,6 +225,11 @@ class GsrSystem:
         ms, cnt = ct.c_double(), ct.c_int64()
         _check(lib().gsr_profile_get(self._h, int(which), ct.byref(ms), ct.byref(cnt)), "gsr_profile_get")
         return ms.value, cnt.value
+
+    def instr_acc_info(self) -> dict:
+        a = (ct.c_int32 * 5)()
+        _check(lib().gsr_instr_acc_info(self._h, a), "gsr_instr_acc_info")
+        return {"two_dies": bool(a[0]), "copies_per_die": a[1], "chunks_per_copy": a[2], "sms_die0": a[3], "sms_die1": a[4]}
 
     def set_option(self, name: str, value: int):
         _check(lib().gsr_set_option(self._h, name.encode(), int(value)), "gsr_set_option")

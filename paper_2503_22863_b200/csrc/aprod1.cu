@@ -132,7 +132,7 @@ static size_t ring_bytes(int w, int st) { return (size_t)w * st * STAGE_BYTES + 
 SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   SmemPlan p;
   p.stages = t.stages > 0 ? t.stages : 2;
-  p.gather_smem = p.acc_smem = false;
+  p.gather_smem = p.acc_smem = p.ins_tab = false;
   const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
   const bool want_acc = (what & PLAN_APROD2) && t.acc_smem, want_gather = (what & PLAN_APROD1) && t.gather_smem;
   const size_t want = (want_acc ? table : 0) + (want_gather ? table : 0);
@@ -146,6 +146,9 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   // privatised accumulators save 6 L2 reductions per row; the gather copy saves 6 L1/L2 gathers per row
   if (want_acc && table <= left) { p.acc_smem = true; left -= table; }
   if (want_gather && table <= left) { p.gather_smem = true; left -= table; }
+  // otherwise the aprod 2 side reduces into die-local chunked copies in L2: room for this CTA's chunk table
+  const size_t tab = ((size_t)((s.I + INS_CHUNK - 1) / INS_CHUNK) * sizeof(double*) + 15) & ~(size_t)15;
+  if ((what & PLAN_APROD2) && !p.acc_smem && tab <= left) { p.ins_tab = true; left -= tab; }
   p.bytes = SMEM_BUDGET - left;
   return p;
 }

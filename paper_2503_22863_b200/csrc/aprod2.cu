@@ -7,7 +7,7 @@ namespace gsr {
 template <bool ASMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
-             double* __restrict__ x, double* __restrict__ gatt_il, double* ins_copies, int n_copies,
+             double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab,
              const double* __restrict__ yscale, const int* done) {
   if (done && *done) return;
   extern __shared__ char smem_raw[];
@@ -16,6 +16,7 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
+  double** tab_s = reinterpret_cast<double**>(acc_s);   // (only one of the two is in use)
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
@@ -23,9 +24,11 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   if (ASMEM) {
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
     __syncthreads();
+  } else if (use_tab) {
+    load_ins_tab(tab_s, ia);
+    __syncthreads();
   }
-  ScatterCtx sc{x, gatt_il, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : x + s.oI,
-                acc_s};
+  ScatterCtx sc{x, gatt_il, x + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr};
   const AttLane al(lane);
   const double ys = yscale ? *yscale : 1.0;
   double gacc = 0.0;
@@ -68,17 +71,18 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   }
 }
 
-// x_instr[i] += sum_c copies[c][i]; copies are cleared for the next call.
+// x_instr[i] += sum over every set (die, copy) of the chunked accumulators; they are cleared for the next call.
 // (The instrumental accumulator is replicated when it does not fit shared memory: 60,000 addresses
 //  hit by 3e9 reductions are contention-bound at L2 -- 159 vs 193 Gadd/s measured with >= 6e5 addresses.)
-__global__ void __launch_bounds__(256) k_fold_instr(double* __restrict__ xins, double* __restrict__ copies, int n_copies,
-                                                    int64_t I, const int* done) {
+__global__ void __launch_bounds__(256) k_fold_instr(double* __restrict__ xins, InstrAcc ia, int64_t I, const int* done) {
   if (done && *done) return;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < I; i += (int64_t)gridDim.x * blockDim.x) {
     double sum = 0.0;
-    for (int c = 0; c < n_copies; c++) {
-      sum += copies[(size_t)c * I + i];
-      copies[(size_t)c * I + i] = 0.0;
+    const int64_t ch = i >> INS_CHUNK_SHIFT, off = i & (INS_CHUNK - 1);
+    for (int c = 0; c < ia.n_sets; c++) {
+      double* p = ia.chunk_tab[(size_t)c * ia.n_chunks + ch] + off;
+      sum += *p;
+      *p = 0.0;
     }
     xins[i] += sum;
   }
@@ -88,7 +92,7 @@ cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, c
                               int64_t* launches) {
   int64_t b = (s.I + 255) / 256;
   if (b > 148 * 4) b = 148 * 4;
-  k_fold_instr<<<(unsigned)b, 256, 0, st>>>(x + s.oI, sd.ins_copies, sd.n_copies, s.I, done);
+  k_fold_instr<<<(unsigned)b, 256, 0, st>>>(x + s.oI, sd.ins, s.I, done);
   ++*launches;
   return cudaGetLastError();
 }
@@ -153,9 +157,11 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
     auto k = p.acc_smem ? k_aprod2_tma<true> : k_aprod2_tma<false>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
-    const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
-    k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc,
-                                            use_copies ? sd.ins_copies : nullptr, sd.n_copies, yscale, done);
+    const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
+    InstrAcc ia = sd.ins;
+    if (!t.die_local) ia.two_dies = false;
+    k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc, ia,
+                                            use_copies ? 1 : 0, yscale, done);
     ++*launches;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

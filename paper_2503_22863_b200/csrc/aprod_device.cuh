@@ -42,6 +42,12 @@ __device__ __forceinline__ double ld_nc_na(const double* p) {
 #endif
 }
 
+// fp64 reduction at L2, fire and forget.  Explicitly .global: a pointer that was read from a table in
+// shared memory would otherwise compile to a GENERIC atomic (no RED, address-space check per lane).
+__device__ __forceinline__ void red_add(double* p, double v) {
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
 // What a kernel needs to gather from x (aprod 1 side).
 struct GatherCtx {
   const double* x;          // the n-vector being multiplied (astro block at x, 5 per star)
@@ -161,8 +167,8 @@ __device__ __forceinline__ void att_scatter(const char* tile, const AttLane& L, 
   if (L.act) {
 #pragma unroll
     for (int it = 0; it < 16; it++)
-      atomicAdd(gatt_il + 3 * (int64_t)t[it] + L.p,
-                *reinterpret_cast<const double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p));
+      red_add(gatt_il + 3 * (int64_t)t[it] + L.p,
+              *reinterpret_cast<const double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p));
   }
 }
 
@@ -192,8 +198,9 @@ __device__ __forceinline__ double row_dot_rest(const RowRegs& r, const GatherCtx
 struct ScatterCtx {
   double* x;        // the n-vector being accumulated into (astro and global parts)
   double* gatt_il;  // attitude accumulator, interleaved layout, 3K doubles
-  double* xins;     // instrumental accumulator in global memory: x + oI, or this CTA's private copy
+  double* xins;     // instrumental accumulator in global memory when neither of the next two is used: x + oI
   double* acc_s;    // shared-memory instrumental accumulator, or nullptr
+  double* const* ins_tab;   // shared-memory table of this CTA's die-local 4 KB accumulator chunks, or nullptr
 };
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -229,13 +236,13 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
     c1 += d1;
     if (q <= s1 - s0 && i < 3) {
       double* xa = x + 5 * (int64_t)(s0 + q) + 2 * i;
-      atomicAdd(xa, c0);
-      if (i < 2) atomicAdd(xa + 1, c1);
+      red_add(xa, c0);
+      if (i < 2) red_add(xa + 1, c1);
     }
   } else if (valid) {
     double* xa = x + 5 * (int64_t)r.i0.x;
 #pragma unroll
-    for (int k = 0; k < 5; k++) atomicAdd(xa + k, r.a[k] * yv);
+    for (int k = 0; k < 5; k++) red_add(xa + k, r.a[k] * yv);
   }
 }
 
@@ -253,9 +260,18 @@ __device__ __forceinline__ double scatter_rest(const RowRegs& r, bool valid, dou
     double inc[6];
 #pragma unroll
     for (int q = 0; q < 6; q++) inc[q] = r.a[17 + q] * yv;
-    double* t = INSTR_SMEM ? c.acc_s : c.xins;
+    if (!INSTR_SMEM && c.ins_tab) {
 #pragma unroll
-    for (int q = 0; q < 6; q++) atomicAdd(t + col[q], inc[q]);
+      for (int q = 0; q < 6; q++) red_add(c.ins_tab[col[q] >> INS_CHUNK_SHIFT] + (col[q] & (INS_CHUNK - 1)), inc[q]);
+    } else {
+      if (INSTR_SMEM) {
+#pragma unroll
+        for (int q = 0; q < 6; q++) atomicAdd(c.acc_s + col[q], inc[q]);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 6; q++) red_add(c.xins + col[q], inc[q]);
+      }
+    }
     gl = r.a[23] * yv;
   }
   return gl;
@@ -266,10 +282,22 @@ struct SmemPlan {
   int warps, stages;
   bool gather_smem;   // instrumental slice of x staged in shared memory (aprod 1 side)
   bool acc_smem;      // instrumental accumulators privatised in shared memory (aprod 2 side)
+  bool ins_tab;       // else: room reserved for the table of die-local accumulator chunks (InstrAcc)
   size_t bytes;       // dynamic shared memory to request
 };
 enum { PLAN_APROD1 = 1, PLAN_APROD2 = 2, PLAN_FUSED = 3 };
 SmemPlan plan_smem(const SysView& s, const Tuning& t, int what);
+
+// This CTA's set of die-local accumulator chunks -> shared memory (n_chunks pointers).  Call before a
+// __syncthreads().  The set is chosen by the die of the SM the CTA runs on.
+__device__ __forceinline__ void load_ins_tab(double** tab_s, const InstrAcc& ia) {
+  unsigned smid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  int die = smid < (unsigned)SMID_SLOTS ? ia.sm_die[smid] : 0;
+  if (die < 0 || !ia.two_dies) die = 0;
+  const int set = die * ia.copies_per_die + (int)(blockIdx.x % (unsigned)ia.copies_per_die);
+  for (int i = threadIdx.x; i < ia.n_chunks; i += blockDim.x) tab_s[i] = ia.chunk_tab[(size_t)set * ia.n_chunks + i];
+}
 
 __device__ __forceinline__ char* smem_align128(char* p) { return p + ((128u - (smem_u32(p) & 127u)) & 127u); }
 

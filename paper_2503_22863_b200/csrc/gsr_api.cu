@@ -1,6 +1,7 @@
 // C ABI of libgsr (include/gsr.h): argument checking, ownership, the LSQR driver.
 // Every step of the path runs in the kernels of aprod1.cu / aprod2.cu / lsqr_kernels.cu.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -102,18 +103,102 @@ static int build_att_buffers(gsr_system* s) {
   return GSR_OK;
 }
 
-// Replicated instrumental accumulators in global memory (L2-resident): one per CTA while that stays
-// under 4 MB, at least 8 (60,000 addresses hit by 3e9 reductions are contention-bound otherwise).
+// ---- die-local replicated instrumental accumulators (InstrAcc, gsr_internal.cuh) ------------------
+// probe_homes: which die is the L2 home of each 4 KB chunk of the pool, and on which die does each SM sit?
+// Thread 0 of every block times a short chain of dependent fp64 atomics (add 0.0) to each of N_REF
+// reference chunks: the latencies fall into two groups, ~330 and ~720 cycles on B200 (near / far die).
+// Die 0 is DEFINED as the home of reference chunk 0; an SM that sees that chunk near sits on die 0.  The
+// block then classifies its share of the pool the same way.  A wrong call only costs speed, never
+// correctness: every chunk is a valid accumulator whoever reduces into it.
+constexpr int N_REF = 16;
+__device__ __forceinline__ float atom_latency(double* p, int reps) {
+  double v;
+  asm volatile("atom.global.add.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "d"(0.0) : "memory");   // warm
+  const long long t0 = clock64();
+  for (int r = 0; r < reps; r++) {
+    double* q = p + (long long)(v * 0.0);   // address depends on the previous result: a serial chain
+    asm volatile("atom.global.add.f64 %0, [%1], %2;" : "=d"(v) : "l"(q), "d"(0.0) : "memory");
+  }
+  const long long t1 = clock64();
+  return (float)(t1 - t0) / (float)reps + (float)(v * 0.0);
+}
+__global__ void k_probe_homes(double* pool, int n_pool, int* sm_die, signed char* home, int* bimodal) {
+  if (threadIdx.x != 0) return;
+  unsigned smid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  float ref[N_REF], srt[N_REF];
+  const int off = (int)((blockIdx.x * 4u) % INS_CHUNK);   // own sector of every reference chunk: no same-address contention
+  for (int c = 0; c < N_REF; c++) atom_latency(pool + (size_t)c * INS_CHUNK + off, 2);   // untimed pass: TLB, first touch
+  for (int c = 0; c < N_REF; c++) srt[c] = ref[c] = atom_latency(pool + (size_t)c * INS_CHUNK + off, 8);
+  for (int i = 1; i < N_REF; i++)   // insertion sort; the threshold is the middle of the widest gap
+    for (int j = i; j > 0 && srt[j] < srt[j - 1]; j--) { const float t = srt[j]; srt[j] = srt[j - 1]; srt[j - 1] = t; }
+  int g = 1;
+  for (int i = 2; i < N_REF; i++)
+    if (srt[i] - srt[i - 1] > srt[g] - srt[g - 1]) g = i;
+  if (srt[g] < 1.4f * srt[g - 1]) { atomicAnd(bimodal, 0); return; }   // no two groups seen from this SM: one die (or an unknown part)
+  const float thr = 0.5f * (srt[g] + srt[g - 1]);
+  const int my_die = ref[0] < thr ? 0 : 1;
+  if (smid < (unsigned)SMID_SLOTS) sm_die[smid] = my_die;
+  for (int c = blockIdx.x; c < n_pool; c += gridDim.x) {
+    const bool near_ = atom_latency(pool + (size_t)c * INS_CHUNK, 8) < thr;
+    home[c] = (signed char)(near_ ? my_die : 1 - my_die);
+  }
+}
+
+// Copies per die: enough that a copy is shared by few CTAs (60,000 addresses hit by 3e9 reductions are
+// contention-bound otherwise), within ~4 MB in total, at least 4 per die.
 static int build_instr_copies(gsr_system* s) {
   const SysView& v = s->v;
-  int64_t copies = (int64_t)(4u << 20) / (v.I * 8);
-  if (copies > s->num_sms) copies = s->num_sms;
-  if (copies < 8) copies = 8;
-  cudaError_t e = cudaMalloc(&s->side.ins_copies, (size_t)copies * v.I * sizeof(double));
-  if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc ins_copies"); }
-  e = cudaMemset(s->side.ins_copies, 0, (size_t)copies * v.I * sizeof(double));
-  if (e != cudaSuccess) return cuda_fail(e, "cudaMemset ins_copies");
-  s->side.n_copies = (int)copies;
+  InstrAcc& ia = s->side.ins;
+  int64_t cpd = (int64_t)(2u << 20) / (v.I * 8);   // (1 to 16 MB per die measured the same at C4)
+  if (cpd > s->num_sms / 2) cpd = s->num_sms / 2;
+  if (cpd < 4) cpd = 4;
+  const int64_t n_chunks = (v.I + INS_CHUNK - 1) / INS_CHUNK;
+  const int64_t need = 2 * cpd * n_chunks;
+  const int64_t n_pool = need + need / 4 + 64 + N_REF;
+  const size_t chunk_bytes = INS_CHUNK * sizeof(double);
+  int* bimodal = nullptr;
+  signed char* home = nullptr;
+  cudaError_t e = cudaMalloc(&ia.pool, (size_t)(n_pool + 1) * chunk_bytes);
+  if (e == cudaSuccess) e = cudaMalloc(&ia.sm_die, SMID_SLOTS * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&ia.chunk_tab, (size_t)need * sizeof(double*));
+  if (e == cudaSuccess) e = cudaMalloc(&home, (size_t)n_pool);
+  if (e == cudaSuccess) e = cudaMalloc(&bimodal, sizeof(int));
+  if (e != cudaSuccess) { cudaGetLastError(); cudaFree(home); cudaFree(bimodal); return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc instr accumulators"); }
+  double* base = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(ia.pool) + chunk_bytes - 1) / chunk_bytes * chunk_bytes);
+  const int one = 1;
+  e = cudaMemset(ia.pool, 0, (size_t)(n_pool + 1) * chunk_bytes);
+  if (e == cudaSuccess) e = cudaMemset(ia.sm_die, 0xff, SMID_SLOTS * sizeof(int));
+  if (e == cudaSuccess) e = cudaMemset(home, 0, (size_t)n_pool);
+  if (e == cudaSuccess) e = cudaMemcpy(bimodal, &one, sizeof(int), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    k_probe_homes<<<2 * s->num_sms, 32>>>(base, (int)n_pool, ia.sm_die, home, bimodal);
+    ++s->launches;
+    e = cudaGetLastError();
+  }
+  std::vector<signed char> h((size_t)n_pool);
+  int two = 0;
+  if (e == cudaSuccess) e = cudaMemcpy(h.data(), home, (size_t)n_pool, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(&two, bimodal, sizeof(int), cudaMemcpyDeviceToHost);
+  cudaFree(home);
+  cudaFree(bimodal);
+  if (e != cudaSuccess) return cuda_fail(e, "probe_homes");
+  // sets 0 .. cpd-1: chunks homed on die 0; sets cpd .. 2 cpd-1: die 1 (a die that runs short borrows from the other)
+  std::vector<int64_t> by_die[2];
+  for (int64_t c = N_REF; c < n_pool; c++) by_die[two ? (h[(size_t)c] != 0) : (c & 1)].push_back(c);
+  std::vector<double*> tab((size_t)need);
+  size_t take[2] = {0, 0};
+  for (int d = 0; d < 2; d++)
+    for (int64_t k = 0; k < cpd * n_chunks; k++) {
+      int src = take[d] < by_die[d].size() ? d : 1 - d;
+      tab[(size_t)(d * cpd * n_chunks + k)] = base + (size_t)by_die[src][take[src]++] * INS_CHUNK;
+    }
+  e = cudaMemcpy(ia.chunk_tab, tab.data(), (size_t)need * sizeof(double*), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpy chunk table");
+  ia.copies_per_die = (int)cpd;
+  ia.n_chunks = (int)n_chunks;
+  ia.two_dies = two != 0;
+  ia.n_sets = (int)(2 * cpd);   // with one die, load_ins_tab uses sets 0 .. cpd-1 only; the others stay zero
   return GSR_OK;
 }
 
@@ -174,7 +259,7 @@ static void free_events(gsr_system* s) {
 extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
-  cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins_copies); cudaFree(s->g);
+  cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins.pool); cudaFree(s->side.ins.sm_die); cudaFree(s->side.ins.chunk_tab); cudaFree(s->g);
   free_events(s);
   delete s;
 }
@@ -466,6 +551,20 @@ extern "C" int gsr_profile_get(gsr_system* s, int which, double* mean_ms, int64_
   return GSR_OK;
 }
 
+extern "C" int gsr_instr_acc_info(const gsr_system* s, int32_t* info) {
+  if (!s || !info) return GSR_EINVAL;
+  const InstrAcc& ia = s->side.ins;
+  std::vector<int> d(SMID_SLOTS, -1);
+  if (ia.sm_die && cudaMemcpy(d.data(), ia.sm_die, SMID_SLOTS * sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return cuda_fail(cudaGetLastError(), "cudaMemcpy sm_die");
+  info[0] = ia.two_dies ? 1 : 0;
+  info[1] = ia.copies_per_die;
+  info[2] = ia.n_chunks;
+  info[3] = info[4] = 0;
+  for (int v : d) { if (v == 0) info[3]++; else if (v == 1) info[4]++; }
+  return GSR_OK;
+}
+
 extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   if (!s || !name) return GSR_EINVAL;
   if (!strcmp(name, "aprod1_variant")) s->tune.aprod1_variant = (int)value;
@@ -475,6 +574,7 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "stages")) s->tune.stages = (int)value;
   else if (!strcmp(name, "instr_copies")) s->tune.instr_copies = (int)value;
   else if (!strcmp(name, "acc_smem")) s->tune.acc_smem = (int)value;
+  else if (!strcmp(name, "die_local")) s->tune.die_local = (int)value;
   else if (!strcmp(name, "gather_smem")) s->tune.gather_smem = (int)value;
   else if (!strcmp(name, "fused")) s->tune.fused = (int)value;
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;

@@ -43,7 +43,26 @@ struct Tuning {
   int instr_copies = 1;    // replicate the instrumental accumulator in global memory when it cannot be privatised
   int fused = 1;           // LSQR: one fused pass over the matrix per iteration (lsqr_fused.cu)
   int acc_smem = 1;        // instrumental accumulators: 1 = privatised in shared memory when they fit, 0 = always L2 copies
+  int die_local = 1;       // L2 instrumental accumulators: 1 = each CTA reduces into a copy homed on its own die, 0 = die-0 copies for all (control)
   int gather_smem = 1;     // instrumental slice of x: 1 = staged in shared memory when it fits, 0 = L1/L2 gathers
+};
+
+// Replicated instrumental accumulators for systems whose slice does not fit shared memory.
+// B200 is two dies; an fp64 reduction executes in the L2 slice that is the HOME of its address, and the
+// home die of an address is a hash of its physical 4 KB granule.  Measured on this part (gsr_api.cu,
+// probe_homes): an atomic to a near-die granule returns in ~330 cycles, to a far-die granule in ~720, and a
+// far reduction costs a second L2 tag lookup on the way (`lts__t_requests_srcunit_ltcfabric`).  So the
+// accumulators are built from 4 KB chunks (512 doubles) whose home die was probed at gsr_create, one set of
+// copies per die, and every CTA reduces into a copy homed on the die its SM sits on.
+constexpr int INS_CHUNK = 512;        // doubles per chunk (4 KB granule)
+constexpr int INS_CHUNK_SHIFT = 9;
+constexpr int SMID_SLOTS = 1024;      // entries of the SM-id -> die table
+struct InstrAcc {
+  double** chunk_tab = nullptr;  // device: [n_sets][n_chunks] chunk pointers; set = die * copies_per_die + copy
+  int* sm_die = nullptr;         // device: [SMID_SLOTS] die (0 / 1) of an SM id
+  void* pool = nullptr;          // device: the chunk pool (zero between calls)
+  int copies_per_die = 0, n_chunks = 0, n_sets = 0;   // n_sets = 2 * copies_per_die (copies_per_die if one die was seen)
+  bool two_dies = false;
 };
 
 // Side structures owned by the library (built in gsr_create).
@@ -51,8 +70,7 @@ struct SideData {
   CUtensorMap map;         // 48 x floor(M/2) fp64 tensor (row pairs), box 50 x 16 (tma.cuh)
   double* att_il = nullptr;   // 3K: interleaved copy of x's attitude block (standalone aprod 1)
   double* att_acc = nullptr;  // 3K: interleaved attitude accumulator, zero between calls (standalone aprod 2)
-  double* ins_copies = nullptr;  // n_copies x I zero-initialised accumulators (only when I*8 exceeds smem)
-  int n_copies = 0;
+  InstrAcc ins;               // die-local replicated instrumental accumulators (global memory, L2-resident)
 };
 
 #ifndef GSR_MAX_TMA_WARPS

@@ -16,7 +16,7 @@ namespace gsr {
 template <bool GSMEM, bool ASMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
-             double* __restrict__ uh, double* __restrict__ g, double* ins_copies, int n_copies,
+             double* __restrict__ uh, double* __restrict__ g, InstrAcc ia, int use_tab,
              const double* __restrict__ c0p, double* usq, int* done) {
   {
     const int d = *done;
@@ -32,6 +32,7 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
   double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : 0);
+  double** tab_s = reinterpret_cast<double**>(xi_s + (GSMEM ? ((s.I + 1) & ~1ll) : 0));
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
@@ -40,11 +41,11 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
   if (GSMEM)
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(v + s.oI + i);
-  if (ASMEM || GSMEM) __syncthreads();
+  if (!ASMEM && use_tab) load_ins_tab(tab_s, ia);
+  if (ASMEM || GSMEM || use_tab) __syncthreads();
   const double* att_il = v + s.oA;
   GatherCtx gc{v, att_il, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
-  ScatterCtx sc{g, g + s.oA, (!ASMEM && ins_copies) ? ins_copies + (size_t)(blockIdx.x % n_copies) * s.I : g + s.oI,
-                acc_s};
+  ScatterCtx sc{g, g + s.oA, g + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr};
   const AttLane al(lane);
   const double c0 = *c0p;
   double sq = 0.0, gacc = 0.0;
@@ -108,15 +109,16 @@ cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning
   const SmemPlan p = plan_smem(s, t, PLAN_FUSED);
   if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
   const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
-  const bool use_copies = !p.acc_smem && sd.ins_copies != nullptr && t.instr_copies != 0;
-  double* copies = use_copies ? sd.ins_copies : nullptr;
-  void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, double*, int, const double*, double*, int*);
+  const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
+  void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, InstrAcc, int, const double*, double*, int*);
   if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true> : k_lsqr_fused<true, false>;
   else k = p.acc_smem ? k_lsqr_fused<false, true> : k_lsqr_fused<false, false>;
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
   if (e != cudaSuccess) return e;
   ++*launches;
-  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, copies, sd.n_copies, c0, usq, done);
+  InstrAcc ia = sd.ins;
+  if (!t.die_local) ia.two_dies = false;
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, ia, use_copies ? 1 : 0, c0, usq, done);
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (use_copies) return launch_fold_instr(s, sd, g, done, st, launches);

@@ -169,6 +169,33 @@ def test_aprod_accumulates():
         assert np.array_equal(y2.cpu().numpy(), once)
 
 
+def test_die_local_instrumental_accumulators():
+    """I = 60,000 cannot be privatised in shared memory: the reductions go to L2-resident copies built from
+    4 KB chunks whose home die gsr_create probed.  Parity must hold with and without die-locality, and on a
+    two-die part (B200) the probe must place every SM on one of the two dies."""
+    shape = C5.scaled(1500, n_knots=4000, n_instr=60_000, n_constraint_rows=50)
+    a, idx = host.make_rows(shape)
+    with make_gpu_system(shape, a, idx) as s:
+        info = s.instr_acc_info()
+        assert info["chunks_per_copy"] == (60_000 + 511) // 512 and info["copies_per_die"] >= 4
+        if info["two_dies"]:
+            props = torch.cuda.get_device_properties(0)
+            assert info["sms_die0"] + info["sms_die1"] == props.multi_processor_count
+            assert min(info["sms_die0"], info["sms_die1"]) >= props.multi_processor_count // 4
+        for die_local in (1, 0):
+            s.set_option("die_local", die_local)
+            check_aprod2(shape, a, idx, s, seed=31 + die_local)
+            check_aprod2(shape, a, idx, s, seed=41 + die_local)      # the copies were cleared by the fold
+        # the fused LSQR pass reduces into the same copies: one-step replays through the oracle (reading R16)
+        b = rhs(shape, a, idx, host.x_true(shape))
+        for die_local in (1, 0):
+            s.set_option("die_local", die_local)
+            s.lsqr_init(dev(b))
+            for k in (0, 2):
+                s.lsqr_iterate(k)
+                replay_one_step(shape, a, idx, s)
+
+
 def test_empty_system_and_errors():
     shape = tiny_shape(n_stars=2, obs=3, n_knots=8, n_instr=6)
     a, idx = host.make_rows(shape)
