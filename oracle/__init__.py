@@ -111,6 +111,10 @@ def lib():
         L.orc_lsqr.restype = ct.c_int
         L.orc_lsqr.argtypes = [LP, ct.c_int64, _dp, _ip, _dp, _dp, ct.c_int64, ct.c_double,
                                ct.c_double, ct.c_double, ct.c_int, ct.POINTER(LsqrResult), _dp, _dp]
+        L.orc_colnorm2.restype = None
+        L.orc_colnorm2.argtypes = [LP, ct.c_int64, _dp, _ip, _dp]
+        L.orc_scale_columns.restype = None
+        L.orc_scale_columns.argtypes = [LP, ct.c_int64, _dp, _ip, _dp, _dp]
         L.orc_max_threads.restype = ct.c_int
         SP = ct.POINTER(_CState)
         L.orc_lsqr_init.restype = None
@@ -214,6 +218,54 @@ def lsqr(L, a, idx, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1, histor
         k = out["itn"] + 1
         return x, out, rh[:k], ah[:k]
     return x, out
+
+
+def colnorms(L, a, idx):
+    """2-norm of every column of A; 0 for a column no row touches."""
+    m = _check(L, a, idx)
+    sq = np.zeros(n_unknowns(L), dtype=np.float64)
+    lib().orc_colnorm2(ct.byref(L), m, _d(a), _i(idx), _d(sq))
+    return np.sqrt(sq)
+
+
+def scale_columns(L, a, idx, s):
+    """The coefficient records of A diag(s)."""
+    m = _check(L, a, idx)
+    out = np.empty_like(a)
+    lib().orc_scale_columns(ct.byref(L), m, _d(a), _i(idx), _d(np.ascontiguousarray(s, dtype=np.float64)), _d(out))
+    return out
+
+
+def lsqr_var(L, a, idx, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1):
+    """LSQR that also returns Paige-Saunders' `var` (the diagonal of (A^T A)^-1 as estimated by the run):
+    var += (w / rho)^2 at every iteration, with the w BEFORE its update and rho of that iteration's plane
+    rotation, rho = sqrt(rhobar_old^2 + beta_new^2).  Written over lsqr_init / lsqr_step, so the LSQR
+    arithmetic itself is the pinned one.  Returns (x, var, result dict)."""
+    st = lsqr_init(L, a, idx, b, threads=threads)
+    var = np.zeros_like(st.x)
+    if st.arnorm == 0.0:
+        st.istop = 0
+    elif itnlim <= 0:
+        st.istop = 7
+    else:
+        while st.istop == 0:
+            w_old, rhobar_old = st.w.copy(), st.rhobar
+            lsqr_step(L, a, idx, st, itnlim=itnlim, atol=atol, btol=btol, conlim=conlim, threads=threads)
+            rho = np.sqrt(rhobar_old * rhobar_old + st.beta * st.beta)
+            var += (w_old / rho) ** 2
+    res = st.scalars()
+    res.update(r1norm=st.rnorm, r2norm=st.rnorm)
+    return st.x.copy(), var, res
+
+
+def lsqr_precond(L, a, idx, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1):
+    """Column-norm preconditioned solve (R7): d = column 2-norms (1 where a column is empty),
+    LSQR on (A D^-1) z = b, x = D^-1 z, var_x = D^-2 var_z.  Returns (x, var, result dict, d)."""
+    d = colnorms(L, a, idx)
+    d[d == 0.0] = 1.0
+    dinv = 1.0 / d
+    z, var_z, res = lsqr_var(L, scale_columns(L, a, idx, dinv), idx, b, itnlim, atol, btol, conlim, threads)
+    return z * dinv, var_z * dinv * dinv, res, d
 
 
 def lsqr_init(L, a, idx, b, threads=1) -> LsqrState:

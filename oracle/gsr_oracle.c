@@ -104,6 +104,27 @@ void orc_aprod1_abs(const orc_layout *L, int64_t nrows, const double *a, const i
 }
 
 /* ------------------------------------------------------------------ OpenMP variants */
+/* the steps either side of the LSQR loop in the paper's solver (PAPER.md:56,
+ * 61, 63: "preconditioned" system, variances of the solution).  The paper gives no formulas; the
+ * reading taken (R7) is diagonal column scaling by the column 2-norms.
+ * nrm2sq[j] = sum_r a[r][k]^2 over the (r,k) with col(r,k) = j : squared 2-norm of column j. */
+void orc_colnorm2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, double *nrm2sq) {
+  for (int64_t r = 0; r < nrows; r++)
+    for (int k = 0; k < NSLOT; k++) {
+      int64_t c = orc_col(L, idx + r * NIDX, k);
+      if (c >= 0) nrm2sq[c] += a[r * NSLOT + k] * a[r * NSLOT + k];
+    }
+}
+/* a_out[r][k] = a[r][k] * s[col(r,k)] : the matrix A diag(s), same index records. */
+void orc_scale_columns(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, const double *s,
+                       double *a_out) {
+  for (int64_t r = 0; r < nrows; r++)
+    for (int k = 0; k < NSLOT; k++) {
+      int64_t c = orc_col(L, idx + r * NIDX, k);
+      a_out[r * NSLOT + k] = c >= 0 ? a[r * NSLOT + k] * s[c] : a[r * NSLOT + k];
+    }
+}
+
 static int clamp_threads(int threads) {
   int mx = orc_max_threads();
   if (threads < 1) threads = 1;

@@ -61,6 +61,12 @@ void orc_aprod2_comp(const orc_layout *L, int64_t nrows, const double *a, const 
 void orc_aprod1_abs(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                     const double *x, const double *y_in, double *s);
 
+/* Column scaling (R7): squared column 2-norms (accumulated into nrm2sq, n),
+ * and a_out = A diag(s) with the same index records. */
+void orc_colnorm2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, double *nrm2sq);
+void orc_scale_columns(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, const double *s,
+                       double *a_out);
+
 /* OpenMP variants (timed CPU baseline; deterministic for a fixed thread count). */
 void orc_aprod1_omp(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                     const double *x, double *y, int threads);
