@@ -141,6 +141,23 @@ int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int
                   const double *b_host, double *x_host, int64_t itnlim, double atol, double btol,
                   double conlim, gsr_lsqr_result *res);
 
+/* ---- the steps either side of the LSQR loop in the paper's solver -------------
+ * PAPER.md:56 "the system is preconditioned", "the variances of the solution are computed /
+ * the solution and its errors are de-preconditioned".  The paper gives no formulas; the reading taken
+ * (R7) is diagonal column scaling: D = diag(||A e_j||_2), 1 for a column no row touches; LSQR runs
+ * on (A D^-1) z = b and returns x = D^-1 z.  The variances are Paige-Saunders' estimate of diag((A^T A)^-1),
+ * var += (w / rho)^2 at every iteration, returned in the units of x (var_x = D^-2 var_z).
+ *
+ * gsr_colnorms : out[j] = ||A e_j||_2 for every unknown (device, n, the ABI's column order), one pass over A.
+ * gsr_lsqr_ex  : gsr_lsqr with `var` (device, n, overwritten; NULL = not wanted) and `flags`
+ *                (GSR_PRECOND_COLNORM or 0).  The norms in `res` are those of the system LSQR iterated on
+ *                (the scaled one when preconditioned), as in the paper's loop.  Errors as gsr_lsqr;
+ *                GSR_ESTATE if the two-pass schedule (option fused=0) is combined with preconditioning. */
+#define GSR_PRECOND_COLNORM 1
+int gsr_colnorms(gsr_system *sys, double *out, void *stream);
+int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_t flags, int64_t itnlim,
+                double atol, double btol, double conlim, gsr_lsqr_result *res, void *stream);
+
 /* ---- diagnostics ----------------------------------------------------------------------------
  * gsr_launch_count : kernels launched by this system object so far (host out-pointer).
  * gsr_profile      : enable (1) / disable (0) CUDA-event timing of the matrix-pass kernels issued by

@@ -50,6 +50,8 @@ class LsqrResult:
     bnorm: float
 
 
+GSR_PRECOND_COLNORM = 1
+
 _lib = None
 
 # name -> (restype, argtypes); every symbol include/gsr.h declares
@@ -61,6 +63,9 @@ SYMBOLS = {
     "gsr_aprod2": (ct.c_int, [_vp, _vp, _vp, _vp]),
     "gsr_lsqr": (ct.c_int, [_vp, _vp, _vp, ct.c_int64, ct.c_double, ct.c_double, ct.c_double,
                             ct.POINTER(_Result), _vp]),
+    "gsr_lsqr_ex": (ct.c_int, [_vp, _vp, _vp, _vp, ct.c_int32, ct.c_int64, ct.c_double, ct.c_double, ct.c_double,
+                               ct.POINTER(_Result), _vp]),
+    "gsr_colnorms": (ct.c_int, [_vp, _vp, _vp]),
     "gsr_lsqr_init": (ct.c_int, [_vp, _vp, _vp]),
     "gsr_lsqr_iterate": (ct.c_int, [_vp, ct.c_int64, ct.c_int64, ct.c_double, ct.c_double, ct.c_double, _vp]),
     "gsr_lsqr_result_get": (ct.c_int, [_vp, _vp, ct.POINTER(_Result), _vp]),
@@ -185,6 +190,22 @@ class GsrSystem:
                               _dev_ptr(x, torch.float64, self.n_unknowns, "x"), int(itnlim), float(atol),
                               float(btol), float(conlim), ct.byref(r), _stream()), "gsr_lsqr")
         return _result(r)
+
+    def lsqr_ex(self, b, x, var=None, precond=False, itnlim=0, atol=0.0, btol=0.0, conlim=0.0) -> LsqrResult:
+        import torch
+        r = _Result()
+        _check(lib().gsr_lsqr_ex(self._h, _dev_ptr(b, torch.float64, self.n_rows, "b"),
+                                 _dev_ptr(x, torch.float64, self.n_unknowns, "x"),
+                                 _dev_ptr(var, torch.float64, self.n_unknowns, "var") if var is not None else None,
+                                 GSR_PRECOND_COLNORM if precond else 0, int(itnlim), float(atol), float(btol),
+                                 float(conlim), ct.byref(r), _stream()), "gsr_lsqr_ex")
+        return _result(r)
+
+    def colnorms(self, out):
+        import torch
+        _check(lib().gsr_colnorms(self._h, _dev_ptr(out, torch.float64, self.n_unknowns, "out"), _stream()),
+               "gsr_colnorms")
+        return out
 
     def lsqr_init(self, b):
         import torch

@@ -38,6 +38,9 @@ struct gsr_system {
   double *u = nullptr, *vv = nullptr, *w = nullptr, *x = nullptr, *g = nullptr;
   DevScalars* sc = nullptr;
   bool lsqr_ready = false;   // gsr_lsqr_init has run
+  // column-norm preconditioning and variances (gsr_lsqr_ex); buffers allocated on first use
+  double *dinv = nullptr, *vs = nullptr, *var = nullptr;   // D^-1, D^-1 v (the vector the matrix pass gathers), var
+  bool opt_precond = false, opt_var = false;               // options of the run set up by the last lsqr init
   // profiling
   bool profile = false;
   std::vector<EventPair> pending;
@@ -260,6 +263,7 @@ extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
   cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins.pool); cudaFree(s->side.ins.sm_die); cudaFree(s->side.ins.chunk_tab); cudaFree(s->g);
+  cudaFree(s->dinv); cudaFree(s->vs); cudaFree(s->var);
   free_events(s);
   delete s;
 }
@@ -335,10 +339,31 @@ static int ensure_workspace(gsr_system* s) {
   return GSR_OK;
 }
 
+// D^-1 (internal layout): one pass over A for the squared column norms, then 1/sqrt with the empty-column guard.
+static int build_dinv(gsr_system* s, cudaStream_t st) {
+  const size_t n = (size_t)s->v.n;
+  if (!s->dinv) CU(cudaMalloc(&s->dinv, n * sizeof(double)));
+  if (!s->vs) CU(cudaMalloc(&s->vs, n * sizeof(double)));
+  CU(cudaMemsetAsync(s->dinv, 0, n * sizeof(double), st));
+  CU(lsqr_launch_colnorm2(s->v, s->dinv, st, &s->launches));
+  CU(lsqr_launch_colnorm_finish(s->dinv, s->v.n, 1, st, &s->launches));
+  return GSR_OK;
+}
+
+static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool want_var, void* stream);
+
 extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
+  return lsqr_init_with(s, b, false, false, stream);
+}
+
+static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool want_var, void* stream) {
   if (!s || (!b && s->v.M > 0)) return GSR_EINVAL;
   int rc = ensure_workspace(s);
   if (rc) return rc;
+  s->opt_precond = precond;
+  s->opt_var = want_var;
+  if (precond && (rc = build_dinv(s, S(stream)))) return rc;
+  if (want_var && !s->var) CU(cudaMalloc(&s->var, (size_t)s->v.n * sizeof(double)));
   cudaStream_t st = S(stream);
   const int64_t M = s->v.M, n = s->v.n;
   CU(cudaMemsetAsync(s->sc, 0, sizeof(DevScalars), st));
@@ -347,9 +372,11 @@ extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
   CU(lsqr_launch_init_s1(s->sc, st, &s->launches));                      // beta
   rc = do_aprod2(s, s->u, s->vv, true, &s->sc->s_y, nullptr, st);        // v = A^T u
   if (rc) return rc;
-  CU(lsqr_launch_sumsq_v(s->vv, n, s->sc, st, &s->launches));
+  const double* dinv = s->opt_precond ? s->dinv : nullptr;               // v = (A D^-1)^T u = D^-1 (A^T u)
+  CU(lsqr_launch_sumsq_v(s->vv, n, s->sc, dinv, st, &s->launches));
   CU(lsqr_launch_init_s2(s->sc, st, &s->launches));                      // alpha and the rest
-  CU(lsqr_launch_init_vw(s->vv, s->w, s->x, n, s->sc, st, &s->launches));
+  CU(lsqr_launch_init_vw(s->vv, s->w, s->x, n, s->sc, s->opt_precond ? s->vs : nullptr, dinv,
+                         s->opt_var ? s->var : nullptr, st, &s->launches));
   s->lsqr_ready = true;
   return GSR_OK;
 }
@@ -361,20 +388,24 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
   cudaStream_t st = S(stream);
   const int64_t n = s->v.n;
   DevScalars* sc = s->sc;
+  const double* dinv = s->opt_precond ? s->dinv : nullptr;
+  double* vs = s->opt_precond ? s->vs : nullptr;          // the matrix pass gathers D^-1 v
+  double* var = s->opt_var ? s->var : nullptr;
+  if (s->opt_precond && !s->tune.fused) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
   for (int64_t it = 0; it < n_iters && s->tune.fused; ++it) {
     // 1+2 in one pass over A: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2 ; g = A^T u_hat
     CU(cudaMemsetAsync(s->g, 0, (size_t)n * sizeof(double), st));
     EventPair ep;
     const bool p = prof_begin(s, 3, st, &ep);
-    cudaError_t e = launch_lsqr_fused(s->v, s->side, s->tune, s->num_sms, s->vv, s->u, s->g, &sc->c0_u, &sc->usq,
-                                      &sc->done, st, &s->launches);
+    cudaError_t e = launch_lsqr_fused(s->v, s->side, s->tune, s->num_sms, vs ? vs : s->vv, s->u, s->g, &sc->c0_u,
+                                      &sc->usq, &sc->done, st, &s->launches);
     if (p) prof_end(s, st, &ep);
     if (e != cudaSuccess) return cuda_fail(e, "fused LSQR pass launch");
     // beta ; v <- g / beta - beta v ; vsq = ||v||^2
-    CU(lsqr_launch_vcombine(s->vv, s->g, n, sc, st, &s->launches));
+    CU(lsqr_launch_vcombine(s->vv, s->g, n, sc, dinv, st, &s->launches));
     // 3-8: scalars, stopping rule ; then the x / w / v update
     CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
-    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, st, &s->launches));
+    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, vs, dinv, var, st, &s->launches));
   }
   for (int64_t it = 0; it < n_iters && !s->tune.fused; ++it) {
     // 1: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2              (aprod 1)
@@ -384,10 +415,10 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
     CU(lsqr_launch_vscale(s->vv, n, sc, st, &s->launches));
     rc = do_aprod2(s, s->u, s->vv, true, &sc->s_y, &sc->done, st);
     if (rc) return rc;
-    CU(lsqr_launch_sumsq_v(s->vv, n, sc, st, &s->launches));
+    CU(lsqr_launch_sumsq_v(s->vv, n, sc, nullptr, st, &s->launches));
     // 3-8: scalars, stopping rule ; then the x / w / v update
     CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
-    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, st, &s->launches));
+    CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, nullptr, nullptr, var, st, &s->launches));
   }
   return GSR_OK;
 }
@@ -419,7 +450,14 @@ extern "C" int gsr_lsqr_result_get(gsr_system* s, double* x_out, gsr_lsqr_result
   if (!s->lsqr_ready) return GSR_ESTATE;
   cudaStream_t st = S(stream);
   int rc;
-  if (x_out && (rc = export_nvec(s, s->x, x_out, st))) return rc;
+  if (x_out) {
+    const double* src = s->x;
+    if (s->opt_precond) {   // x = D^-1 z (g is free between iterations)
+      CU(lsqr_launch_scale_by(s->g, s->x, s->dinv, s->v.n, 1, st, &s->launches));
+      src = s->g;
+    }
+    if ((rc = export_nvec(s, src, x_out, st))) return rc;
+  }
   DevScalars h;
   rc = fetch_scalars(s, &h, st);
   if (rc) return rc;
@@ -452,8 +490,25 @@ extern "C" int gsr_lsqr_get_state(gsr_system* s, double* u, double* v, double* w
 
 extern "C" int gsr_lsqr(gsr_system* s, const double* b, double* x, int64_t itnlim, double atol,
                         double btol, double conlim, gsr_lsqr_result* res, void* stream) {
-  if (!s || !x || !res || itnlim < 0) return GSR_EINVAL;
-  int rc = gsr_lsqr_init(s, b, stream);
+  return gsr_lsqr_ex(s, b, x, nullptr, 0, itnlim, atol, btol, conlim, res, stream);
+}
+
+extern "C" int gsr_colnorms(gsr_system* s, double* out, void* stream) {
+  if (!s || !out) return GSR_EINVAL;
+  int rc = ensure_workspace(s);
+  if (rc) return rc;
+  cudaStream_t st = S(stream);
+  CU(cudaMemsetAsync(s->g, 0, (size_t)s->v.n * sizeof(double), st));
+  CU(lsqr_launch_colnorm2(s->v, s->g, st, &s->launches));
+  CU(lsqr_launch_colnorm_finish(s->g, s->v.n, 0, st, &s->launches));
+  return export_nvec(s, s->g, out, st);
+}
+
+extern "C" int gsr_lsqr_ex(gsr_system* s, const double* b, double* x, double* var, int32_t flags, int64_t itnlim,
+                           double atol, double btol, double conlim, gsr_lsqr_result* res, void* stream) {
+  if (!s || !x || !res || itnlim < 0 || (flags & ~GSR_PRECOND_COLNORM)) return GSR_EINVAL;
+  if ((flags & GSR_PRECOND_COLNORM) && !s->tune.fused) return GSR_ESTATE;
+  int rc = lsqr_init_with(s, b, (flags & GSR_PRECOND_COLNORM) != 0, var != nullptr, stream);
   if (rc) return rc;
   cudaStream_t st = S(stream);
   DevScalars h;
@@ -469,6 +524,14 @@ extern "C" int gsr_lsqr(gsr_system* s, const double* b, double* x, int64_t itnli
     if ((rc = gsr_lsqr_iterate(s, batch, itnlim, atol, btol, conlim, stream))) return rc;
     issued += batch;
     if ((rc = fetch_scalars(s, &h, st))) return rc;   // poll the device-side stop flag
+  }
+  if (var) {   // var_x = D^-2 var_z (g is free between iterations)
+    const double* src = s->var;
+    if (s->opt_precond) {
+      CU(lsqr_launch_scale_by(s->g, s->var, s->dinv, s->v.n, 2, st, &s->launches));
+      src = s->g;
+    }
+    if ((rc = export_nvec(s, src, var, st))) return rc;
   }
   return gsr_lsqr_result_get(s, x, res, stream);
 }

@@ -28,6 +28,7 @@ struct DevScalars {
   double c0_u;                   // aprod1 fused update: u_hat <- A v + c0_u * u_hat  (= -alpha/beta)
   double s_y;                    // aprod2 input scale (1/beta: u = u_hat / beta is never stored)
   double t1, t2, inv_alpha;      // x/w/v update coefficients of the current iteration
+  double inv_rho;                // 1 / rho of the current plane rotation (variance update)
   long long itn;
   int istop;
   int done;                      // 1 once a stopping rule fired: later kernels are no-ops
@@ -101,18 +102,26 @@ cudaError_t launch_att_from_il(const SysView& s, int num_sms, const double* il, 
                                int64_t* launches);
 cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, const int* done, cudaStream_t st,
                               int64_t* launches);
-cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, const double* dinv,
+                                 cudaStream_t st, int64_t* launches);
 
 // LSQR vector / scalar kernels (lsqr_kernels.cu)
 cudaError_t lsqr_launch_init_u(const double* b, double* u, int64_t M, DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launches);
-cudaError_t lsqr_launch_sumsq_v(const double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_sumsq_v(double* v, int64_t n, DevScalars* sc, const double* dinv, cudaStream_t st,
+                                int64_t* launches);
 cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches);
-cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
+                                const double* dinv, double* var, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
                                      cudaStream_t st, int64_t* launches);
-cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
+                               const double* dinv, double* var, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_colnorm2(const SysView& s, double* d2, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s, int64_t n, int power, cudaStream_t st,
+                                 int64_t* launches);
 cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches);
 
 // ---- device helpers -----------------------------------------------------------------------

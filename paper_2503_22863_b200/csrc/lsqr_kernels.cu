@@ -44,12 +44,15 @@ __global__ void k_init_s1(DevScalars* sc) {
   sc->itn = 0;
 }
 
-__global__ void __launch_bounds__(256) k_sumsq_v(const double* __restrict__ v, int64_t n, DevScalars* sc) {
+// vsq = ||v||^2; with a preconditioner, v <- D^-1 v first (v = A^T u becomes (A D^-1)^T u)
+__global__ void __launch_bounds__(256) k_sumsq_v(double* __restrict__ v, int64_t n, DevScalars* sc,
+                                                 const double* __restrict__ dinv) {
   if (sc->done) return;
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
        i += (int64_t)gridDim.x * blockDim.x) {
-    const double t = v[i];
+    double t = v[i];
+    if (dinv) { t *= dinv[i]; v[i] = t; }
     sq = fma(t, t, sq);
   }
   sq = block_sum(sq);
@@ -74,8 +77,11 @@ __global__ void k_init_s2(DevScalars* sc) {
 }
 
 // v /= alpha ; w = v ; x = 0 ; wsq = ||w||^2                                         (init)
+// (vs = D^-1 v is what the matrix pass gathers when a preconditioner is on; var starts at 0)
 __global__ void __launch_bounds__(256) k_init_vw(double* __restrict__ v, double* __restrict__ w,
-                                                 double* __restrict__ x, int64_t n, DevScalars* sc) {
+                                                 double* __restrict__ x, int64_t n, DevScalars* sc,
+                                                 double* __restrict__ vs, const double* __restrict__ dinv,
+                                                 double* __restrict__ var) {
   const double ia = sc->inv_alpha;
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
@@ -84,6 +90,8 @@ __global__ void __launch_bounds__(256) k_init_vw(double* __restrict__ v, double*
     v[i] = t;
     w[i] = t;
     x[i] = 0.0;
+    if (vs) vs[i] = t * dinv[i];
+    if (var) var[i] = 0.0;
     sq = fma(t, t, sq);
   }
   sq = block_sum(sq);
@@ -109,8 +117,9 @@ __global__ void __launch_bounds__(256) k_vscale(double* __restrict__ v, int64_t 
 
 // fused path, step 2: beta = ||u_hat||; v <- g / beta - beta v (un-normalised v'), vsq = ||v'||^2.
 // g = A^T u_hat was accumulated by the fused pass.  Thread 0 publishes beta, 1/beta and anorm.
+// With a preconditioner g holds A^T u_hat and the operator's transpose is D^-1 A^T: g is scaled on the fly.
 __global__ void __launch_bounds__(256) k_vcombine(double* __restrict__ v, const double* __restrict__ g, int64_t n,
-                                                  DevScalars* sc) {
+                                                  DevScalars* sc, const double* __restrict__ dinv) {
   if (sc->done) return;
   const double beta = sqrt(sc->usq);
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -123,7 +132,8 @@ __global__ void __launch_bounds__(256) k_vcombine(double* __restrict__ v, const 
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
        i += (int64_t)gridDim.x * blockDim.x) {
-    const double t = fma(nb, v[i], g[i] * ib);
+    const double gi = dinv ? g[i] * dinv[i] : g[i];
+    const double t = fma(nb, v[i], gi * ib);
     v[i] = t;
     sq = fma(t, t, sq);
   }
@@ -149,6 +159,7 @@ __global__ void k_step_scalars(DevScalars* sc, int64_t itnlim, double atol, doub
   // 4: coefficients of the x / w update; ||w/rho||^2 = wsq / rho^2
   sc->t1 = phi / rho;
   sc->t2 = -theta / rho;
+  sc->inv_rho = 1.0 / rho;
   sc->ddnorm += sc->wsq / (rho * rho);
   // 5: ||x|| estimate
   const double delta = sc->sn2 * rho, gambar = -sc->cs2 * rho, rhs = phi - delta * sc->z;
@@ -191,15 +202,20 @@ __global__ void k_step_scalars(DevScalars* sc, int64_t itnlim, double atol, doub
 }
 
 // step 4 (vectors): v /= alpha ; x += t1 w ; w = v + t2 w ; wsq = ||w_new||^2
+// optional: var += (w_old / rho)^2 (Paige-Saunders' variance estimate); vs = D^-1 v (preconditioned gather vector)
 __global__ void __launch_bounds__(256) k_update(double* __restrict__ v, double* __restrict__ w,
-                                                double* __restrict__ x, int64_t n, DevScalars* sc) {
+                                                double* __restrict__ x, int64_t n, DevScalars* sc,
+                                                double* __restrict__ vs, const double* __restrict__ dinv,
+                                                double* __restrict__ var) {
   if (sc->done == 1) return;
-  const double ia = sc->inv_alpha, t1 = sc->t1, t2 = sc->t2;
+  const double ia = sc->inv_alpha, t1 = sc->t1, t2 = sc->t2, ir = sc->inv_rho;
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
        i += (int64_t)gridDim.x * blockDim.x) {
     const double vi = v[i] * ia, wi = w[i];
     v[i] = vi;
+    if (vs) vs[i] = vi * dinv[i];
+    if (var) { const double dk = ir * wi; var[i] = fma(dk, dk, var[i]); }
     x[i] = fma(t1, wi, x[i]);
     const double wn = fma(t2, wi, vi);
     w[i] = wn;
@@ -228,24 +244,27 @@ cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launch
   k_init_s1<<<1, 1, 0, st>>>(sc);
   return LAUNCHED();
 }
-cudaError_t lsqr_launch_sumsq_v(const double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
-  k_sumsq_v<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc);
+cudaError_t lsqr_launch_sumsq_v(double* v, int64_t n, DevScalars* sc, const double* dinv, cudaStream_t st,
+                                int64_t* launches) {
+  k_sumsq_v<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc, dinv);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches) {
   k_init_s2<<<1, 1, 0, st>>>(sc);
   return LAUNCHED();
 }
-cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
-  k_init_vw<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc);
+cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
+                                const double* dinv, double* var, cudaStream_t st, int64_t* launches) {
+  k_init_vw<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
   k_vscale<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc);
   return LAUNCHED();
 }
-cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
-  k_vcombine<<<grid_for(n, 256, 4), 256, 0, st>>>(v, g, n, sc);
+cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, const double* dinv,
+                                 cudaStream_t st, int64_t* launches) {
+  k_vcombine<<<grid_for(n, 256, 4), 256, 0, st>>>(v, g, n, sc, dinv);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
@@ -253,8 +272,70 @@ cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol
   k_step_scalars<<<1, 1, 0, st>>>(sc, itnlim, atol, btol, conlim);
   return LAUNCHED();
 }
-cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
-  k_update<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc);
+cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
+                               const double* dinv, double* var, cudaStream_t st, int64_t* launches) {
+  k_update<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var);
+  return LAUNCHED();
+}
+
+// ---- column norms and the diagonal preconditioner (reading R7) ----------
+// d2[col(r,k)] += a[r][k]^2 for every stored coefficient; d2 is an LSQR-internal n-vector (attitude block
+// interleaved, il[3*t + ax]).  One pass over A at gsr_lsqr_ex / gsr_colnorms time, not part of the iteration:
+// one thread per row, fp64 reductions at L2.
+__global__ void __launch_bounds__(256) k_colnorm2(SysView s, double* __restrict__ d2) {
+  for (int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; r < s.M; r += (int64_t)gridDim.x * blockDim.x) {
+    const double2* ap = reinterpret_cast<const double2*>(s.vals + r * NSLOT);
+    const int4* ip = reinterpret_cast<const int4*>(s.idx + r * NIDX);
+    const int4 i0 = __ldg(ip), i1 = __ldg(ip + 1);
+    double a[NSLOT];
+#pragma unroll
+    for (int q = 0; q < NSLOT / 2; q++) {
+      const double2 t = __ldcs(ap + q);
+      a[2 * q] = t.x;
+      a[2 * q + 1] = t.y;
+    }
+    double* xa = d2 + 5 * (int64_t)i0.x;
+#pragma unroll
+    for (int k = 0; k < 5; k++) atomicAdd(xa + k, a[k] * a[k]);
+    double* xt = d2 + s.oA + 3 * (int64_t)i0.y;
+#pragma unroll
+    for (int ax = 0; ax < 3; ax++)
+#pragma unroll
+      for (int j = 0; j < 4; j++) atomicAdd(xt + 3 * j + ax, a[5 + 4 * ax + j] * a[5 + 4 * ax + j]);
+    double* xi = d2 + s.oI;
+    const int col[6] = {i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+#pragma unroll
+    for (int q = 0; q < 6; q++) atomicAdd(xi + col[q], a[17 + q] * a[17 + q]);
+    if (s.G) atomicAdd(d2 + s.oG, a[23] * a[23]);
+  }
+}
+// mode 0: d <- sqrt(d2) (column norms); mode 1: d <- 1 / sqrt(d2), 1 for a column no row touches (D^-1)
+__global__ void __launch_bounds__(256) k_colnorm_finish(double* __restrict__ d, int64_t n, int mode) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double q = sqrt(d[i]);
+    d[i] = mode == 0 ? q : (q > 0.0 ? 1.0 / q : 1.0);
+  }
+}
+// dst = src * s (power 1) or src * s^2 (power 2): x = D^-1 z, var_x = D^-2 var_z
+__global__ void __launch_bounds__(256) k_scale_by(double* __restrict__ dst, const double* __restrict__ src,
+                                                  const double* __restrict__ s, int64_t n, int power) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double f = s[i];
+    dst[i] = src[i] * (power == 2 ? f * f : f);
+  }
+}
+cudaError_t lsqr_launch_colnorm2(const SysView& s, double* d2, cudaStream_t st, int64_t* launches) {
+  if (s.M == 0) return cudaSuccess;
+  k_colnorm2<<<grid_for(s.M, 256, 1), 256, 0, st>>>(s, d2);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches) {
+  k_colnorm_finish<<<grid_for(n, 256, 4), 256, 0, st>>>(d, n, mode);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s, int64_t n, int power, cudaStream_t st,
+                                 int64_t* launches) {
+  k_scale_by<<<grid_for(n, 256, 4), 256, 0, st>>>(dst, src, s, n, power);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches) {
