@@ -1,4 +1,6 @@
 // aprod2:  x[col(r,k)] += a[r][k] * (yscale * y[r])                  (Eq. 3)
+// square = 1:  x[col(r,k)] += a[r][k]^2  (squared column norms: the same pass with the
+//              coefficients squared on the fly and y = 1; y may be null)
 #include "aprod_device.cuh"
 
 namespace gsr {
@@ -8,7 +10,7 @@ template <bool ASMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
              double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab,
-             const double* __restrict__ yscale, const int* done) {
+             const double* __restrict__ yscale, const int* done, int square) {
   if (done && *done) return;
   extern __shared__ char smem_raw[];
   char* smem = smem_align128(smem_raw);
@@ -33,7 +35,7 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   const double ys = yscale ? *yscale : 1.0;
   double gacc = 0.0;
 
-  double ynext = (gw < ring.n_tiles && gw * TILE_ROWS + lane < s.M) ? y[gw * TILE_ROWS + lane] : 0.0;
+  double ynext = (!square && gw < ring.n_tiles && gw * TILE_ROWS + lane < s.M) ? y[gw * TILE_ROWS + lane] : 1.0;
   for (int64_t t = gw; t < ring.n_tiles; t += W) {
     const int64_t row0 = t * TILE_ROWS;
     const int64_t r = row0 + lane;
@@ -41,19 +43,23 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const double yv = valid ? ys * ynext : 0.0;
     {  // prefetch the next tile's y
       const int64_t rn = r + W * TILE_ROWS;
-      ynext = rn < s.M ? y[rn] : 0.0;
+      if (!square) ynext = rn < s.M ? y[rn] : 0.0;
     }
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     char* tile = ring.acquire(t, lane);
     RowRegs row;
     load_row(tile, lane, valid, row);
+    if (square) {
+#pragma unroll
+      for (int k = 0; k < NSLOT; k++) row.a[k] *= row.a[k];
+    }
     int ts[16];
     att_starts(tile, al, ts);
     __syncwarp();   // every lane holds its row: the exchange runs may be written
     att_products(tile, lane, row, yv);
     __syncwarp();
     att_scatter(tile, al, ts, gatt_il);
-    astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x);
+    astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x, square != 0);
     gacc += scatter_rest<ASMEM>(row, valid, yv, sc);
     ring.release(lane);
   }
@@ -148,9 +154,9 @@ __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const doubl
 // otherwise the attitude products go to the zeroed side buffer sd.att_acc and are folded into x.
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
                           double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
-                          int64_t* launches) {
+                          int64_t* launches, int square) {
   if (s.M == 0) return cudaSuccess;
-  if (t.aprod2_variant == 1) {
+  if (t.aprod2_variant == 1 || square) {
     const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
@@ -161,7 +167,7 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
     InstrAcc ia = sd.ins;
     if (!t.die_local) ia.two_dies = false;
     k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc, ia,
-                                            use_copies ? 1 : 0, yscale, done);
+                                            use_copies ? 1 : 0, yscale, done, square);
     ++*launches;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

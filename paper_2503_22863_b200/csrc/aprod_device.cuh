@@ -217,8 +217,9 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // at most 2 reductions.  Exact fp64 FMAs (the indicator multiplies by 1 or adds 0).
 // Otherwise (stars with < 5 rows, or unused star ids inside the tile): 5 reductions per row.
 // Requires: att_products(yv) stored (yv = 0 for rows past the end) and a __syncwarp() since.
+// square: the staged coefficients are squared on the fly (column-norm pass; r.a is squared by the caller).
 __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nvalid, bool valid, const RowRegs& r,
-                                              double yv, double* __restrict__ x) {
+                                              double yv, double* __restrict__ x, bool square = false) {
   const int s0 = __shfl_sync(FULL, r.i0.x, 0), s1 = __shfl_sync(FULL, r.i0.x, nvalid - 1);
   if (s1 - s0 < 8) {
     const int q = lane >> 2, i = lane & 3;
@@ -228,7 +229,8 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
       const int row = 4 * j + i;
       const int st = *reinterpret_cast<const int*>(tile + COEF_TILE_BYTES + row * 32);
       const double y = *reinterpret_cast<const double*>(tile + pad_off(row));
-      const double b = *reinterpret_cast<const double*>(tile + row_off(row) + 8 * (q < 5 ? q : 0));
+      double b = *reinterpret_cast<const double*>(tile + row_off(row) + 8 * (q < 5 ? q : 0));
+      if (square) b *= b;
       if (j & 1) dmma884(d0, d1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
       else dmma884(c0, c1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
     }

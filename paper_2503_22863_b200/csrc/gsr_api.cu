@@ -345,7 +345,7 @@ static int build_dinv(gsr_system* s, cudaStream_t st) {
   if (!s->dinv) CU(cudaMalloc(&s->dinv, n * sizeof(double)));
   if (!s->vs) CU(cudaMalloc(&s->vs, n * sizeof(double)));
   CU(cudaMemsetAsync(s->dinv, 0, n * sizeof(double), st));
-  CU(lsqr_launch_colnorm2(s->v, s->dinv, st, &s->launches));
+  CU(launch_aprod2(s->v, s->side, s->tune, s->num_sms, nullptr, s->dinv, true, nullptr, nullptr, st, &s->launches, 1));
   CU(lsqr_launch_colnorm_finish(s->dinv, s->v.n, 1, st, &s->launches));
   return GSR_OK;
 }
@@ -499,7 +499,7 @@ extern "C" int gsr_colnorms(gsr_system* s, double* out, void* stream) {
   if (rc) return rc;
   cudaStream_t st = S(stream);
   CU(cudaMemsetAsync(s->g, 0, (size_t)s->v.n * sizeof(double), st));
-  CU(lsqr_launch_colnorm2(s->v, s->g, st, &s->launches));
+  CU(launch_aprod2(s->v, s->side, s->tune, s->num_sms, nullptr, s->g, true, nullptr, nullptr, st, &s->launches, 1));
   CU(lsqr_launch_colnorm_finish(s->g, s->v.n, 0, st, &s->launches));
   return export_nvec(s, s->g, out, st);
 }

@@ -89,7 +89,7 @@ cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t,
 //   aprod2: x += A^T (yscale * y)
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
                           double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
-                          int64_t* launches);
+                          int64_t* launches, int square = 0);
 cudaError_t launch_validate(const SysView& s, int* flag, cudaStream_t st, int64_t* launches);
 //   fused LSQR step: uh <- A v + c0 uh ; g += A^T uh ; usq += ||uh||^2   (lsqr_fused.cu; v, g internal layout)
 cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* v,
@@ -118,7 +118,6 @@ cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol
                                      cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
                                const double* dinv, double* var, cudaStream_t st, int64_t* launches);
-cudaError_t lsqr_launch_colnorm2(const SysView& s, double* d2, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s, int64_t n, int power, cudaStream_t st,
                                  int64_t* launches);

@@ -279,36 +279,8 @@ cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevSc
 }
 
 // ---- column norms and the diagonal preconditioner (reading R7) ----------
-// d2[col(r,k)] += a[r][k]^2 for every stored coefficient; d2 is an LSQR-internal n-vector (attitude block
-// interleaved, il[3*t + ax]).  One pass over A at gsr_lsqr_ex / gsr_colnorms time, not part of the iteration:
-// one thread per row, fp64 reductions at L2.
-__global__ void __launch_bounds__(256) k_colnorm2(SysView s, double* __restrict__ d2) {
-  for (int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; r < s.M; r += (int64_t)gridDim.x * blockDim.x) {
-    const double2* ap = reinterpret_cast<const double2*>(s.vals + r * NSLOT);
-    const int4* ip = reinterpret_cast<const int4*>(s.idx + r * NIDX);
-    const int4 i0 = __ldg(ip), i1 = __ldg(ip + 1);
-    double a[NSLOT];
-#pragma unroll
-    for (int q = 0; q < NSLOT / 2; q++) {
-      const double2 t = __ldcs(ap + q);
-      a[2 * q] = t.x;
-      a[2 * q + 1] = t.y;
-    }
-    double* xa = d2 + 5 * (int64_t)i0.x;
-#pragma unroll
-    for (int k = 0; k < 5; k++) atomicAdd(xa + k, a[k] * a[k]);
-    double* xt = d2 + s.oA + 3 * (int64_t)i0.y;
-#pragma unroll
-    for (int ax = 0; ax < 3; ax++)
-#pragma unroll
-      for (int j = 0; j < 4; j++) atomicAdd(xt + 3 * j + ax, a[5 + 4 * ax + j] * a[5 + 4 * ax + j]);
-    double* xi = d2 + s.oI;
-    const int col[6] = {i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
-#pragma unroll
-    for (int q = 0; q < 6; q++) atomicAdd(xi + col[q], a[17 + q] * a[17 + q]);
-    if (s.G) atomicAdd(d2 + s.oG, a[23] * a[23]);
-  }
-}
+// The squared column norms are accumulated by the aprod 2 tile kernel with its coefficients squared on the
+// fly (aprod2.cu, square = 1), into an LSQR-internal n-vector (attitude block interleaved).
 // mode 0: d <- sqrt(d2) (column norms); mode 1: d <- 1 / sqrt(d2), 1 for a column no row touches (D^-1)
 __global__ void __launch_bounds__(256) k_colnorm_finish(double* __restrict__ d, int64_t n, int mode) {
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -323,11 +295,6 @@ __global__ void __launch_bounds__(256) k_scale_by(double* __restrict__ dst, cons
     const double f = s[i];
     dst[i] = src[i] * (power == 2 ? f * f : f);
   }
-}
-cudaError_t lsqr_launch_colnorm2(const SysView& s, double* d2, cudaStream_t st, int64_t* launches) {
-  if (s.M == 0) return cudaSuccess;
-  k_colnorm2<<<grid_for(s.M, 256, 1), 256, 0, st>>>(s, d2);
-  return LAUNCHED();
 }
 cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches) {
   k_colnorm_finish<<<grid_for(n, 256, 4), 256, 0, st>>>(d, n, mode);
