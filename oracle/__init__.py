@@ -258,6 +258,32 @@ def lsqr_var(L, a, idx, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1):
     return st.x.copy(), var, res
 
 
+def lsqr_cov(L, a, idx, b, j1, j2, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1):
+    """Covariances of chosen pairs of unknowns, Eq. (4): Cov[p] += factor^itn * x^itn[j1[p]] *
+    x^itn[j2[p]] at every LSQR iteration.  Reading (R21): this is the off-diagonal companion of
+    Paige-Saunders' var, i.e. x^itn is the direction w of that iteration (before its update) and factor^itn =
+    1 / rho^2, so that a pair (j, j) reproduces var[j] and the sum estimates ((A^T A)^-1)[j1, j2].
+    Returns (x, cov, result dict)."""
+    j1 = np.asarray(j1, dtype=np.int64)
+    j2 = np.asarray(j2, dtype=np.int64)
+    st = lsqr_init(L, a, idx, b, threads=threads)
+    cov = np.zeros(j1.shape[0], dtype=np.float64)
+    if st.arnorm == 0.0:
+        st.istop = 0
+    elif itnlim <= 0:
+        st.istop = 7
+    else:
+        while st.istop == 0:
+            w_old, rhobar_old = st.w.copy(), st.rhobar
+            lsqr_step(L, a, idx, st, itnlim=itnlim, atol=atol, btol=btol, conlim=conlim, threads=threads)
+            rho = np.sqrt(rhobar_old * rhobar_old + st.beta * st.beta)
+            for p in range(j1.shape[0]):
+                cov[p] += (1.0 / (rho * rho)) * w_old[j1[p]] * w_old[j2[p]]
+    res = st.scalars()
+    res.update(r1norm=st.rnorm, r2norm=st.rnorm)
+    return st.x.copy(), cov, res
+
+
 def lsqr_precond(L, a, idx, b, itnlim, atol=0.0, btol=0.0, conlim=0.0, threads=1):
     """Column-norm preconditioned solve (R7): d = column 2-norms (1 where a column is empty),
     LSQR on (A D^-1) z = b, x = D^-1 z, var_x = D^-2 var_z.  Returns (x, var, result dict, d)."""

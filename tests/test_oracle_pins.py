@@ -438,3 +438,35 @@ def test_preconditioned_lsqr_gives_the_same_least_squares_solution_in_fewer_iter
     assert np.allclose(oracle.colnorms(L, oracle.scale_columns(L, a, idx, 1.0 / d), idx)[d != 1.0], 1.0, rtol=1e-14)
     keep = nonempty_columns(shape, idx)
     assert np.all(var1[~keep] == 0.0) and np.all(var1[keep] > 0.0)
+
+
+def test_covariances_of_pairs():
+    """Eq. (4) (PAPER.md:86-92), reading R21.  Pins: a pair (j, j) is var[j] (pinned against scipy above);
+    swapping j1 and j2 changes nothing; |cov| <= sqrt(var var) (the estimate is a sum of outer products);
+    and on a single-star, astro-only system (5 unknowns) five iterations span the whole space, so the sum of
+    outer products IS (A^T A)^-1, entry by entry."""
+    shape = tiny_shape(seed=2024)
+    a, idx = host.make_rows(shape)
+    L = oracle.layout_of(shape)
+    b = rhs(shape, a, idx, host.x_true(shape))
+    n = shape.n_unknowns
+    rng = np.random.default_rng(7)
+    j1 = np.concatenate([np.arange(n), rng.integers(0, n, 200)])
+    j2 = np.concatenate([np.arange(n), rng.integers(0, n, 200)])
+    x, cov, res = oracle.lsqr_cov(L, a, idx, b, j1, j2, 15)
+    x2, var, res2 = oracle.lsqr_var(L, a, idx, b, 15)
+    assert np.array_equal(x, x2) and np.allclose(cov[:n], var, rtol=1e-13, atol=0)
+    _, cov_sw, _ = oracle.lsqr_cov(L, a, idx, b, j2, j1, 15)
+    assert np.allclose(cov, cov_sw, rtol=1e-13, atol=1e-18)     # (factor * a) * b vs (factor * b) * a: rounding only
+    assert np.all(np.abs(cov[n:]) <= np.sqrt(var[j1[n:]] * var[j2[n:]]) * (1 + 1e-12))
+    # single star, astro only: a dense 5-column problem
+    one = SystemShape("one", n_stars=1, obs_per_star=40, n_knots=8, n_instr=8, n_glob=1, seed=5)
+    a1, idx1 = host.make_rows(one)
+    a1[:, 5:] = 0.0
+    L1 = oracle.layout_of(one)
+    b1 = host.test_vector(3, 1, a1.shape[0])
+    p1, p2 = np.meshgrid(np.arange(5), np.arange(5), indexing="ij")
+    _, c5, r5 = oracle.lsqr_cov(L1, a1, idx1, b1, p1.ravel(), p2.ravel(), 5)
+    A5 = a1[:, :5]
+    exact = np.linalg.inv(A5.T @ A5)
+    assert r5["itn"] == 5 and np.allclose(c5.reshape(5, 5), exact, rtol=1e-8, atol=1e-10 * np.abs(exact).max())
