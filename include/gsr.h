@@ -153,7 +153,16 @@ int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int
  *                (GSR_PRECOND_COLNORM or 0).  The norms in `res` are those of the system LSQR iterated on
  *                (the scaled one when preconditioned), as in the paper's loop.  Errors as gsr_lsqr;
  *                GSR_ESTATE if the two-pass schedule (option fused=0) is combined with preconditioning. */
+/* gsr_set_cov_pairs : covariances of chosen pairs of unknowns, Eq. (4): Cov[p] += factor^itn *
+ *                x^itn[j1[p]] * x^itn[j2[p]] at every iteration.  Reading (R21): the off-diagonal companion
+ *                of var, x^itn = the direction w of the iteration, factor = 1/rho^2, so a pair (j, j) gives var[j].
+ *                j1, j2 (device, n_pairs x int64, columns in the ABI's order) and cov (device, n_pairs doubles) are
+ *                BORROWED until the next gsr_set_cov_pairs or gsr_destroy; every later gsr_lsqr_ex zeroes cov,
+ *                accumulates into it on the device (the paper's file pipeline between two programs is not needed when
+ *                x lives in one GPU) and returns it in the units of x.  n_pairs = 0 unregisters.
+ *                GSR_EINVAL if an index is outside [0, n). */
 #define GSR_PRECOND_COLNORM 1
+int gsr_set_cov_pairs(gsr_system *sys, const int64_t *j1, const int64_t *j2, int64_t n_pairs, double *cov, void *stream);
 int gsr_colnorms(gsr_system *sys, double *out, void *stream);
 int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_t flags, int64_t itnlim,
                 double atol, double btol, double conlim, gsr_lsqr_result *res, void *stream);

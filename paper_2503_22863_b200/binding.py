@@ -66,6 +66,7 @@ SYMBOLS = {
     "gsr_lsqr_ex": (ct.c_int, [_vp, _vp, _vp, _vp, ct.c_int32, ct.c_int64, ct.c_double, ct.c_double, ct.c_double,
                                ct.POINTER(_Result), _vp]),
     "gsr_colnorms": (ct.c_int, [_vp, _vp, _vp]),
+    "gsr_set_cov_pairs": (ct.c_int, [_vp, _vp, _vp, ct.c_int64, _vp, _vp]),
     "gsr_lsqr_init": (ct.c_int, [_vp, _vp, _vp]),
     "gsr_lsqr_iterate": (ct.c_int, [_vp, ct.c_int64, ct.c_int64, ct.c_double, ct.c_double, ct.c_double, _vp]),
     "gsr_lsqr_result_get": (ct.c_int, [_vp, _vp, ct.POINTER(_Result), _vp]),
@@ -200,6 +201,18 @@ class GsrSystem:
                                  GSR_PRECOND_COLNORM if precond else 0, int(itnlim), float(atol), float(btol),
                                  float(conlim), ct.byref(r), _stream()), "gsr_lsqr_ex")
         return _result(r)
+
+    def set_cov_pairs(self, j1, j2, cov):
+        """Register (or, with j1 = None, unregister) the covariance pairs; the three tensors are borrowed."""
+        import torch
+        if j1 is None:
+            _check(lib().gsr_set_cov_pairs(self._h, None, None, 0, None, _stream()), "gsr_set_cov_pairs")
+            self._cov_refs = None
+            return
+        n = int(j1.numel())
+        _check(lib().gsr_set_cov_pairs(self._h, _dev_ptr(j1, torch.int64, n, "j1"), _dev_ptr(j2, torch.int64, n, "j2"),
+                                       n, _dev_ptr(cov, torch.float64, n, "cov"), _stream()), "gsr_set_cov_pairs")
+        self._cov_refs = (j1, j2, cov)      # keep the borrowed tensors alive
 
     def colnorms(self, out):
         import torch

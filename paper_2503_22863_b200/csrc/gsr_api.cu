@@ -41,6 +41,11 @@ struct gsr_system {
   // column-norm preconditioning and variances (gsr_lsqr_ex); buffers allocated on first use
   double *dinv = nullptr, *vs = nullptr, *var = nullptr;   // D^-1, D^-1 v (the vector the matrix pass gathers), var
   bool opt_precond = false, opt_var = false;               // options of the run set up by the last lsqr init
+  // covariances of chosen pairs (gsr_set_cov_pairs); the three arrays are borrowed
+  const int64_t *cov_j1 = nullptr, *cov_j2 = nullptr;
+  double* cov = nullptr;
+  int64_t n_cov = 0;
+  bool opt_cov = false, opt_cov_next = false;              // (opt_cov_next: set by gsr_lsqr_ex for its own init)
   // profiling
   bool profile = false;
   std::vector<EventPair> pending;
@@ -351,6 +356,8 @@ static int build_dinv(gsr_system* s, cudaStream_t st) {
 }
 
 static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool want_var, void* stream);
+static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int32_t flags, int64_t itnlim, double atol,
+                    double btol, double conlim, gsr_lsqr_result* res, void* stream, bool with_cov);
 
 extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
   return lsqr_init_with(s, b, false, false, stream);
@@ -364,6 +371,8 @@ static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool wan
   s->opt_var = want_var;
   if (precond && (rc = build_dinv(s, S(stream)))) return rc;
   if (want_var && !s->var) CU(cudaMalloc(&s->var, (size_t)s->v.n * sizeof(double)));
+  s->opt_cov = s->opt_cov_next && s->n_cov > 0;
+  if (s->opt_cov) CU(cudaMemsetAsync(s->cov, 0, (size_t)s->n_cov * sizeof(double), S(stream)));
   cudaStream_t st = S(stream);
   const int64_t M = s->v.M, n = s->v.n;
   CU(cudaMemsetAsync(s->sc, 0, sizeof(DevScalars), st));
@@ -405,6 +414,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
     CU(lsqr_launch_vcombine(s->vv, s->g, n, sc, dinv, st, &s->launches));
     // 3-8: scalars, stopping rule ; then the x / w / v update
     CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
+    if (s->opt_cov) CU(lsqr_launch_cov_update(s->v, s->w, sc, s->cov_j1, s->cov_j2, s->n_cov, s->cov, st, &s->launches));
     CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, vs, dinv, var, st, &s->launches));
   }
   for (int64_t it = 0; it < n_iters && !s->tune.fused; ++it) {
@@ -418,6 +428,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
     CU(lsqr_launch_sumsq_v(s->vv, n, sc, nullptr, st, &s->launches));
     // 3-8: scalars, stopping rule ; then the x / w / v update
     CU(lsqr_launch_step_scalars(sc, itnlim, atol, btol, conlim, st, &s->launches));
+    if (s->opt_cov) CU(lsqr_launch_cov_update(s->v, s->w, sc, s->cov_j1, s->cov_j2, s->n_cov, s->cov, st, &s->launches));
     CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, nullptr, nullptr, var, st, &s->launches));
   }
   return GSR_OK;
@@ -490,7 +501,28 @@ extern "C" int gsr_lsqr_get_state(gsr_system* s, double* u, double* v, double* w
 
 extern "C" int gsr_lsqr(gsr_system* s, const double* b, double* x, int64_t itnlim, double atol,
                         double btol, double conlim, gsr_lsqr_result* res, void* stream) {
-  return gsr_lsqr_ex(s, b, x, nullptr, 0, itnlim, atol, btol, conlim, res, stream);
+  return lsqr_run(s, b, x, nullptr, 0, itnlim, atol, btol, conlim, res, stream, false);
+}
+
+extern "C" int gsr_set_cov_pairs(gsr_system* s, const int64_t* j1, const int64_t* j2, int64_t n_pairs, double* cov,
+                                 void* stream) {
+  if (!s || n_pairs < 0) return GSR_EINVAL;
+  if (n_pairs > 0 && (!j1 || !j2 || !cov)) return GSR_EINVAL;
+  s->cov_j1 = s->cov_j2 = nullptr; s->cov = nullptr; s->n_cov = 0;
+  if (n_pairs == 0) return GSR_OK;
+  cudaStream_t st = S(stream);
+  int* bad = nullptr;
+  int h = 0;
+  CU(cudaMalloc(&bad, sizeof(int)));
+  cudaError_t e = cudaMemsetAsync(bad, 0, sizeof(int), st);
+  if (e == cudaSuccess) e = lsqr_launch_check_pairs(j1, j2, n_pairs, s->v.n, bad, st, &s->launches);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(bad);
+  if (e != cudaSuccess) return cuda_fail(e, "gsr_set_cov_pairs");
+  if (h) return GSR_EINVAL;
+  s->cov_j1 = j1; s->cov_j2 = j2; s->cov = cov; s->n_cov = n_pairs;
+  return GSR_OK;
 }
 
 extern "C" int gsr_colnorms(gsr_system* s, double* out, void* stream) {
@@ -506,9 +538,16 @@ extern "C" int gsr_colnorms(gsr_system* s, double* out, void* stream) {
 
 extern "C" int gsr_lsqr_ex(gsr_system* s, const double* b, double* x, double* var, int32_t flags, int64_t itnlim,
                            double atol, double btol, double conlim, gsr_lsqr_result* res, void* stream) {
+  return lsqr_run(s, b, x, var, flags, itnlim, atol, btol, conlim, res, stream, true);
+}
+
+static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int32_t flags, int64_t itnlim, double atol,
+                    double btol, double conlim, gsr_lsqr_result* res, void* stream, bool with_cov) {
   if (!s || !x || !res || itnlim < 0 || (flags & ~GSR_PRECOND_COLNORM)) return GSR_EINVAL;
   if ((flags & GSR_PRECOND_COLNORM) && !s->tune.fused) return GSR_ESTATE;
+  s->opt_cov_next = with_cov;   // gsr_lsqr_ex accumulates the registered covariance pairs; gsr_lsqr / gsr_lsqr_init do not
   int rc = lsqr_init_with(s, b, (flags & GSR_PRECOND_COLNORM) != 0, var != nullptr, stream);
+  s->opt_cov_next = false;
   if (rc) return rc;
   cudaStream_t st = S(stream);
   DevScalars h;
@@ -525,6 +564,8 @@ extern "C" int gsr_lsqr_ex(gsr_system* s, const double* b, double* x, double* va
     issued += batch;
     if ((rc = fetch_scalars(s, &h, st))) return rc;   // poll the device-side stop flag
   }
+  if (s->opt_cov && s->opt_precond)
+    CU(lsqr_launch_cov_unscale(s->v, s->dinv, s->cov_j1, s->cov_j2, s->n_cov, s->cov, st, &s->launches));
   if (var) {   // var_x = D^-2 var_z (g is free between iterations)
     const double* src = s->var;
     if (s->opt_precond) {

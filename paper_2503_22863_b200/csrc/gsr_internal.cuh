@@ -118,6 +118,12 @@ cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol
                                      cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
                                const double* dinv, double* var, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_cov_update(const SysView& s, const double* w, const DevScalars* sc, const int64_t* j1,
+                                   const int64_t* j2, int64_t n_pairs, double* cov, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_cov_unscale(const SysView& s, const double* dinv, const int64_t* j1, const int64_t* j2,
+                                    int64_t n_pairs, double* cov, cudaStream_t st, int64_t* launches);
+cudaError_t lsqr_launch_check_pairs(const int64_t* j1, const int64_t* j2, int64_t n_pairs, int64_t n, int* bad,
+                                    cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s, int64_t n, int power, cudaStream_t st,
                                  int64_t* launches);

@@ -296,6 +296,53 @@ __global__ void __launch_bounds__(256) k_scale_by(double* __restrict__ dst, cons
     dst[i] = src[i] * (power == 2 ? f * f : f);
   }
 }
+// ---- covariances of chosen pairs (Eq. 4; R21) ---------
+// position of API column j inside an LSQR-internal n-vector (attitude block interleaved: il[3*t + ax])
+__device__ __forceinline__ int64_t internal_index(const SysView& s, int64_t j) {
+  if (j < s.oA || j >= s.oI) return j;
+  const int64_t e = j - s.oA, ax = e / s.K, t = e - ax * s.K;
+  return s.oA + 3 * t + ax;
+}
+// cov[p] += (1/rho^2) * w[j1[p]] * w[j2[p]] with the w BEFORE this iteration's update (run before k_update);
+// a gather-multiply-accumulate over the pair list, 24 bytes of list + accumulator traffic per pair.
+__global__ void __launch_bounds__(256) k_cov_update(SysView s, const double* __restrict__ w, const DevScalars* sc,
+                                                    const int64_t* __restrict__ j1, const int64_t* __restrict__ j2,
+                                                    int64_t n_pairs, double* __restrict__ cov) {
+  if (sc->done == 1) return;
+  const double f = sc->inv_rho * sc->inv_rho;
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < n_pairs; p += (int64_t)gridDim.x * blockDim.x)
+    cov[p] = fma(f * __ldg(w + internal_index(s, j1[p])), __ldg(w + internal_index(s, j2[p])), cov[p]);
+}
+// preconditioned run: cov_x = dinv[j1] * dinv[j2] * cov_z
+__global__ void __launch_bounds__(256) k_cov_unscale(SysView s, const double* __restrict__ dinv,
+                                                     const int64_t* __restrict__ j1, const int64_t* __restrict__ j2,
+                                                     int64_t n_pairs, double* __restrict__ cov) {
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < n_pairs; p += (int64_t)gridDim.x * blockDim.x)
+    cov[p] *= __ldg(dinv + internal_index(s, j1[p])) * __ldg(dinv + internal_index(s, j2[p]));
+}
+__global__ void __launch_bounds__(256) k_check_pairs(const int64_t* __restrict__ j1, const int64_t* __restrict__ j2,
+                                                     int64_t n_pairs, int64_t n, int* bad) {
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < n_pairs; p += (int64_t)gridDim.x * blockDim.x)
+    if (j1[p] < 0 || j1[p] >= n || j2[p] < 0 || j2[p] >= n) *bad = 1;
+}
+cudaError_t lsqr_launch_cov_update(const SysView& s, const double* w, const DevScalars* sc, const int64_t* j1,
+                                   const int64_t* j2, int64_t n_pairs, double* cov, cudaStream_t st, int64_t* launches) {
+  if (n_pairs == 0) return cudaSuccess;
+  k_cov_update<<<grid_for(n_pairs, 256, 4), 256, 0, st>>>(s, w, sc, j1, j2, n_pairs, cov);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_cov_unscale(const SysView& s, const double* dinv, const int64_t* j1, const int64_t* j2,
+                                    int64_t n_pairs, double* cov, cudaStream_t st, int64_t* launches) {
+  if (n_pairs == 0) return cudaSuccess;
+  k_cov_unscale<<<grid_for(n_pairs, 256, 4), 256, 0, st>>>(s, dinv, j1, j2, n_pairs, cov);
+  return LAUNCHED();
+}
+cudaError_t lsqr_launch_check_pairs(const int64_t* j1, const int64_t* j2, int64_t n_pairs, int64_t n, int* bad,
+                                    cudaStream_t st, int64_t* launches) {
+  if (n_pairs == 0) return cudaSuccess;
+  k_check_pairs<<<grid_for(n_pairs, 256, 4), 256, 0, st>>>(j1, j2, n_pairs, n, bad);
+  return LAUNCHED();
+}
 cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStream_t st, int64_t* launches) {
   k_colnorm_finish<<<grid_for(n, 256, 4), 256, 0, st>>>(d, n, mode);
   return LAUNCHED();

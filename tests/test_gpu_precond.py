@@ -110,3 +110,44 @@ def test_preconditioned_solve(shape):
         with pytest.raises(Exception):
             s.lsqr_ex(dev(b), x, precond=True, itnlim=2)
         s.set_option("fused", 1)
+
+
+def test_covariances_of_pairs():
+    """SURVEY.md 8(f4), Eq. (4): pairs from every parameter block, plain and preconditioned."""
+    shape = C5.scaled(120, n_knots=90, n_instr=25, n_constraint_rows=20)
+    a, idx = badly_scaled(shape)
+    L = oracle.layout_of(shape)
+    b = rhs(shape, a, idx, host.x_true(shape))
+    n = shape.n_unknowns
+    rng = np.random.default_rng(11)
+    j1 = np.concatenate([np.arange(n), rng.integers(0, n, 3000), rng.integers(shape.off_att, n, 3000)])
+    j2 = np.concatenate([np.arange(n), rng.integers(0, n, 3000), rng.integers(shape.off_att, n, 3000)])
+    with make(shape, a, idx) as s:
+        x = torch.empty(n, dtype=torch.float64, device=DEV)
+        var = torch.empty_like(x)
+        cov = torch.full((j1.size,), 7.0, dtype=torch.float64, device=DEV)        # must be zeroed by the run
+        s.set_cov_pairs(dev(j1), dev(j2), cov)
+        for k in (1, 4):
+            s.lsqr_ex(dev(b), x, var=var, itnlim=k)
+            xo, co, ro = oracle.lsqr_cov(L, a, idx, b, j1, j2, k)
+            cg = cov.cpu().numpy()
+            assert np.linalg.norm(cg - co) <= 1e-9 * np.linalg.norm(co)
+            assert np.linalg.norm(cg[:n] - var.cpu().numpy()) <= 1e-12 * np.linalg.norm(cg[:n])   # pair (j, j) = var[j]
+            # preconditioned: the oracle on the scaled matrix, brought back to the units of x
+            s.lsqr_ex(dev(b), x, precond=True, itnlim=k)
+            d = oracle.colnorms(L, a, idx)
+            d[d == 0.0] = 1.0
+            zo, cz, rz = oracle.lsqr_cov(L, oracle.scale_columns(L, a, idx, 1.0 / d), idx, b, j1, j2, k)
+            cp = cz / (d[j1] * d[j2])
+            assert np.linalg.norm(cov.cpu().numpy() - cp) <= 1e-9 * np.linalg.norm(cp)
+        # a plain gsr_lsqr leaves the registered accumulator alone; unregistering works; bad indices are refused
+        before = cov.clone()
+        s.lsqr(dev(b), x, 3)
+        assert torch.equal(before, cov)
+        bad = j2.copy()
+        bad[5] = n
+        with pytest.raises(Exception):
+            s.set_cov_pairs(dev(j1), dev(bad), cov)
+        s.set_cov_pairs(None, None, None)
+        s.lsqr_ex(dev(b), x, itnlim=2)
+        assert torch.equal(before, cov)
