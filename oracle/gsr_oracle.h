@@ -11,6 +11,12 @@
  *   orc_lsqr   : Paige-Saunders LSQR PAPER.md:35, 41, 53-64 (Sec. 2 solver outline),
  *                refs [29,30] at PAPER.md:234-235; damp = 0, no preconditioning
  *                (reading R7).
+ *   orc_colnorm2, orc_scale_columns, and in oracle/__init__.py lsqr_var / lsqr_precond / lsqr_cov (written over
+ *                orc_lsqr_init / orc_lsqr_step): the steps either side of the loop
+ *                (preconditioning, variances) and PAPER.md:86-92 Eq. 4 (covariances).  The paper gives no
+ *                formulas for these: the readings R7 / R21 of DESIGN.md are what is implemented -- PARITY UNPINNED
+ *                BY THE PAPER for the choice of reading; the functions themselves are pinned (dense matrix,
+ *                scipy's var, (A^T A)^-1, dense least squares).
  * The matrix is the paper's compressed storage: 24 fp64 coefficients per
  * row = 5 astrometric + 12 attitude + 6 instrumental + 1 global; the column of every
  * slot is derived from the 8-int32 index record {star, att_start, instr[6]} as fixed
