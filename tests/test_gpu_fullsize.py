@@ -198,6 +198,28 @@ def test_c4_full_size_aprod_and_lsqr():
         s.aprod1(-x, r)                                   # r = b - A x
         rn = float(torch.linalg.norm(r))
         assert abs(rn - res.r1norm) <= 1e-8 * rn, f"residual identity: {rn} vs {res.r1norm}"
+        del r
+        # SURVEY.md 8(f1) at full size.  Column norms: sum_j ||A e_j||^2 = ||A||_F^2 = the sum of all squared
+        # coefficients (no row repeats a column in this generator), and sampled astrometric columns against
+        # their contiguous rows.  Preconditioned LSQR: the same residual identity in the units of x.
+        cn = torch.empty(n, dtype=torch.float64, device=DEV)
+        s.colnorms(cn)
+        fro2 = 0.0
+        for r0 in range(0, m, 50_000_000):
+            fro2 += float(torch.sum(vals[r0:r0 + 50_000_000] ** 2))
+        assert abs(float(torch.sum(cn * cn)) - fro2) <= 1e-12 * fro2
+        for st in (0, 1234567, shape.n_stars - 1):
+            rows = vals[st * 100:(st + 1) * 100, :5]
+            ref = torch.sqrt(torch.sum(rows * rows, dim=0))
+            assert torch.allclose(cn[5 * st:5 * st + 5], ref, rtol=1e-13, atol=0)
+        var = torch.empty(n, dtype=torch.float64, device=DEV)
+        resp = s.lsqr_ex(b, x, var=var, precond=True, itnlim=10)
+        assert resp.itn == 10 and resp.r1norm < res.r1norm       # column scaling converges faster here
+        r = b.clone()
+        s.aprod1(-x, r)
+        rn = float(torch.linalg.norm(r))
+        assert abs(rn - resp.r1norm) <= 1e-8 * rn, f"preconditioned residual identity: {rn} vs {resp.r1norm}"
+        assert float(var.min()) >= 0.0 and float(var.max()) > 0.0
     finally:
         s.destroy()
         del vals, idx
