@@ -186,6 +186,8 @@ int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_
  *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x
  *                      fused             1 (default) one pass over A per LSQR iteration, 0 aprod 1 then aprod 2
  *                      aprod1_variant, aprod2_variant   1 (default) TMA tiles, 0 one thread per row (cross-check)
+ *                      graph             1 (default) small, launch-bound systems (matrix <= 256 MB): the launches of a batch
+ *                                        of LSQR iterations are captured once into a CUDA graph and replayed, 0 never
  *                      check_every       LSQR iterations between host polls of the stop flag (default 16)      */
 int gsr_launch_count(const gsr_system *sys, int64_t *n_launches);
 int gsr_profile(gsr_system *sys, int enable);

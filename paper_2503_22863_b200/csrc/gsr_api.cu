@@ -27,6 +27,7 @@ struct EventPair {
   int which;
 };
 
+struct IterGraph;
 struct gsr_system {
   SysView v;
   SideData side;
@@ -38,6 +39,8 @@ struct gsr_system {
   double *u = nullptr, *vv = nullptr, *w = nullptr, *x = nullptr, *g = nullptr;
   DevScalars* sc = nullptr;
   bool lsqr_ready = false;   // gsr_lsqr_init has run
+  IterGraph* iter_graph = nullptr;   // cached CUDA graph of a batch of iterations (small systems)
+  cudaStream_t cap_stream = nullptr; // the stream those batches are captured on
   // column-norm preconditioning and variances (gsr_lsqr_ex); buffers allocated on first use
   double *dinv = nullptr, *vs = nullptr, *var = nullptr;   // D^-1, D^-1 v (the vector the matrix pass gathers), var
   bool opt_precond = false, opt_var = false;               // options of the run set up by the last lsqr init
@@ -264,8 +267,11 @@ static void free_events(gsr_system* s) {
   s->pool.clear();
 }
 
+static void free_iter_graph(gsr_system* s);
+
 extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
+  free_iter_graph(s);
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
   cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins.pool); cudaFree(s->side.ins.sm_die); cudaFree(s->side.ins.chunk_tab); cudaFree(s->g);
   cudaFree(s->dinv); cudaFree(s->vs); cudaFree(s->var);
@@ -390,17 +396,14 @@ static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool wan
   return GSR_OK;
 }
 
-extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, double atol, double btol,
-                                double conlim, void* stream) {
-  if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
-  if (!s->lsqr_ready) return GSR_ESTATE;
-  cudaStream_t st = S(stream);
+// Issue the launches of n_iters LSQR iterations on st (eagerly, or into a stream capture).
+static int issue_iterations(gsr_system* s, int64_t n_iters, int64_t itnlim, double atol, double btol, double conlim,
+                            cudaStream_t st) {
   const int64_t n = s->v.n;
   DevScalars* sc = s->sc;
   const double* dinv = s->opt_precond ? s->dinv : nullptr;
   double* vs = s->opt_precond ? s->vs : nullptr;          // the matrix pass gathers D^-1 v
   double* var = s->opt_var ? s->var : nullptr;
-  if (s->opt_precond && !s->tune.fused) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
   for (int64_t it = 0; it < n_iters && s->tune.fused; ++it) {
     // 1+2 in one pass over A: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2 ; g = A^T u_hat
     CU(cudaMemsetAsync(s->g, 0, (size_t)n * sizeof(double), st));
@@ -431,6 +434,91 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
     if (s->opt_cov) CU(lsqr_launch_cov_update(s->v, s->w, sc, s->cov_j1, s->cov_j2, s->n_cov, s->cov, st, &s->launches));
     CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, nullptr, nullptr, var, st, &s->launches));
   }
+  return GSR_OK;
+}
+
+// Small systems are launch-bound: one iteration is a memset and 4-5 kernels, ~39 us at C1 of which the matrix
+// pass is 15 us.  There the launches of a batch of iterations are captured once into a CUDA graph and replayed
+// (the kernels read every iteration-dependent scalar from device memory, so the graph never changes).  The
+// key holds everything that is baked into the captured launches.
+struct IterGraph {
+  cudaGraphExec_t exec = nullptr;
+  int64_t n_iters = 0, itnlim = 0, launches = 0, n_cov = 0;
+  double atol = 0, btol = 0, conlim = 0;
+  int fused = 0, warps = 0, stages = 0, acc_smem = 0, gather_smem = 0, die_local = 0, instr_copies = 0, ctas = 0;
+  int a1v = 0, a2v = 0;
+  bool precond = false, var = false, cov = false;
+  const void *j1 = nullptr, *j2 = nullptr, *covp = nullptr;
+};
+static bool same_key(const IterGraph& a, const IterGraph& b) {
+  return a.n_iters == b.n_iters && a.itnlim == b.itnlim && a.atol == b.atol && a.btol == b.btol && a.conlim == b.conlim &&
+         a.fused == b.fused && a.warps == b.warps && a.stages == b.stages && a.acc_smem == b.acc_smem &&
+         a.gather_smem == b.gather_smem && a.die_local == b.die_local && a.instr_copies == b.instr_copies &&
+         a.ctas == b.ctas && a.a1v == b.a1v && a.a2v == b.a2v && a.precond == b.precond && a.var == b.var &&
+         a.cov == b.cov && a.n_cov == b.n_cov && a.j1 == b.j1 && a.j2 == b.j2 && a.covp == b.covp;
+}
+
+static void free_iter_graph(gsr_system* s) {
+  if (s->iter_graph) {
+    if (s->iter_graph->exec) cudaGraphExecDestroy(s->iter_graph->exec);
+    delete s->iter_graph;
+    s->iter_graph = nullptr;
+  }
+  if (s->cap_stream) { cudaStreamDestroy(s->cap_stream); s->cap_stream = nullptr; }
+}
+
+extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, double atol, double btol,
+                                double conlim, void* stream) {
+  if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
+  if (!s->lsqr_ready) return GSR_ESTATE;
+  if (s->opt_precond && !s->tune.fused) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
+  cudaStream_t st = S(stream);
+  const bool small = (double)s->v.M * 224.0 <= 256.0 * 1024 * 1024;
+  if (!s->tune.graph || s->profile || n_iters < 2 || !small)
+    return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
+  IterGraph key;
+  key.n_iters = n_iters; key.itnlim = itnlim; key.atol = atol; key.btol = btol; key.conlim = conlim;
+  key.fused = s->tune.fused; key.warps = s->tune.warps; key.stages = s->tune.stages; key.acc_smem = s->tune.acc_smem;
+  key.gather_smem = s->tune.gather_smem; key.die_local = s->tune.die_local; key.instr_copies = s->tune.instr_copies;
+  key.ctas = s->tune.ctas_per_sm; key.a1v = s->tune.aprod1_variant; key.a2v = s->tune.aprod2_variant;
+  key.precond = s->opt_precond; key.var = s->opt_var; key.cov = s->opt_cov; key.n_cov = s->n_cov;
+  key.j1 = s->cov_j1; key.j2 = s->cov_j2; key.covp = s->cov;
+  IterGraph* g = s->iter_graph;
+  if (g && g->exec && same_key(*g, key)) {
+    CU(cudaGraphLaunch(g->exec, st));
+    s->launches += g->launches;
+    return GSR_OK;
+  }
+  if (!g) g = s->iter_graph = new (std::nothrow) IterGraph();
+  if (!g) return GSR_ENOMEM;
+  if (g->exec) { cudaGraphExecDestroy(g->exec); g->exec = nullptr; }
+  const int64_t before = s->launches;
+  // captured on a stream of our own (the caller's may be the legacy default stream, which cannot capture;
+  // nothing executes during a capture, so no ordering with st is needed); the graph is launched into st
+  if (!s->cap_stream) CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+  CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+  const int rc = issue_iterations(s, n_iters, itnlim, atol, btol, conlim, s->cap_stream);
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
+  if (rc != GSR_OK || e != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    s->launches = before;
+    if (rc != GSR_OK) return rc;
+    return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);   // capture refused: run eagerly
+  }
+  cudaGraphExec_t exec = nullptr;
+  e = cudaGraphInstantiate(&exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    s->launches = before;
+    return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
+  }
+  *g = key;
+  g->exec = exec;
+  g->launches = s->launches - before;      // what one replay launches (counted once by the capture itself)
+  CU(cudaGraphLaunch(exec, st));
   return GSR_OK;
 }
 
@@ -679,6 +767,7 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "instr_copies")) s->tune.instr_copies = (int)value;
   else if (!strcmp(name, "acc_smem")) s->tune.acc_smem = (int)value;
   else if (!strcmp(name, "die_local")) s->tune.die_local = (int)value;
+  else if (!strcmp(name, "graph")) s->tune.graph = (int)value;
   else if (!strcmp(name, "gather_smem")) s->tune.gather_smem = (int)value;
   else if (!strcmp(name, "fused")) s->tune.fused = (int)value;
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;

@@ -43,6 +43,7 @@ struct Tuning {
   int check_every = 16;    // LSQR iterations between host polls of the stop flag
   int instr_copies = 1;    // replicate the instrumental accumulator in global memory when it cannot be privatised
   int fused = 1;           // LSQR: one fused pass over the matrix per iteration (lsqr_fused.cu)
+  int graph = 1;           // LSQR: replay batches of iterations of small (launch-bound) systems as a CUDA graph
   int acc_smem = 1;        // instrumental accumulators: 1 = privatised in shared memory when they fit, 0 = always L2 copies
   int die_local = 1;       // L2 instrumental accumulators: 1 = each CTA reduces into a copy homed on its own die, 0 = die-0 copies for all (control)
   int gather_smem = 1;     // instrumental slice of x: 1 = staged in shared memory when it fits, 0 = L1/L2 gathers
