@@ -24,23 +24,9 @@ namespace gsr {
 
 constexpr unsigned FULL = 0xffffffffu;
 
-// streaming (single-use) 8-byte gather: do not allocate in L1 (keeps L1 for the instrumental slice)
-#ifndef ATT_LD_MODE
-#define ATT_LD_MODE 1
-#endif
-__device__ __forceinline__ double ld_nc_na(const double* p) {
-#if ATT_LD_MODE == 0
-  double v;
-  asm("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
-  return v;
-#elif ATT_LD_MODE == 1
-  return __ldg(p);
-#elif ATT_LD_MODE == 2
-  return *p;
-#else
-  return 1.0 + (double)(reinterpret_cast<uintptr_t>(p) & 8);   // experiment: no load at all
-#endif
-}
+// 8-byte gather through the read-only path (measured the same with L1::no_allocate, with plain ld.global and
+// with an L2 evict-last policy on the attitude table: profiles/r01_summary.md section 3)
+__device__ __forceinline__ double ld_nc_na(const double* p) { return __ldg(p); }
 
 // fp64 reduction at L2, fire and forget.  Explicitly .global: a pointer that was read from a table in
 // shared memory would otherwise compile to a GENERIC atomic (no RED, address-space check per lane).
