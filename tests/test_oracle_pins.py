@@ -17,6 +17,19 @@ from gaia_synth.configs import C1, SystemShape
 from helpers import (columns_of, csr_matrix, dense_matrix, nonempty_columns, rhs, tiny_shape)
 
 
+def _read_golden(name):
+    """tests/golden/<name>: lines `key v v v ...` (ints; `|` separators ignored), repeated keys accumulate."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)) as f:
+        for ln in f:
+            ln = ln.split("#")[0].strip()
+            if ln:
+                k, *v = ln.replace("|", " ").split()
+                out.setdefault(k, []).append([int(t) for t in v])
+    return out
+
+
 def _sys(shape):
     a, idx = host.make_rows(shape)
     return a, idx, oracle.layout_of(shape)
@@ -43,22 +56,27 @@ def test_hand_worked_two_rows():
     aprod2 with y = (1, 2), x0 = 0: x[26] = a0 part (slots 19 and 22 -> 1+1)*1 + 117*2 = 236;
       x[28] = 1*1 + 23*2 = 47; x[0] = 1; x[9] = 4*2 = 8; x[11] = row0 slot5 (1) + row1 slot6 (6*2) = 13.
     """
-    L = oracle.layout(2, 5, 3, 1)
+    g = _read_golden("two_rows.txt")
+    S, K, I, G = g["layout"][0]
+    L = oracle.layout(S, K, I, G)
     assert oracle.n_unknowns(L) == 29
-    a = np.ones((2, 24))
-    a[1] = np.arange(24)
-    idx = np.array([[0, 1, 0, 2, 1, 0, 2, 1], [1, 0, 1, 1, 1, 1, 1, 1]], dtype=np.int32)
+    idx = np.array([r[:8] for r in g["row"]], dtype=np.int32)
+    a = np.array([r[8:] for r in g["row"]], dtype=np.float64)
+    assert a.shape == (2, 24) and a[1].tolist() == list(range(24))
     x = np.arange(1, 30, dtype=np.float64)
     y = oracle.aprod1(L, a, idx, x, np.zeros(2))
-    assert y.tolist() == [428.0, 6296.0]
+    assert y.tolist() == [float(v) for v in g["aprod1_y"][0]]
     x2 = oracle.aprod2(L, a, idx, np.array([1.0, 2.0]), np.zeros(29))
-    assert x2[26] == 236.0 and x2[28] == 47.0 and x2[0] == 1.0 and x2[9] == 8.0 and x2[11] == 13.0
+    for j, v in g["aprod2_x"]:
+        assert x2[j] == float(v)
     # n_glob = 0: slot 23 is ignored and x has 28 entries
-    L0 = oracle.layout(2, 5, 3, 0)
+    L0 = oracle.layout(S, K, I, 0)
     y0 = oracle.aprod1(L0, a, idx, x[:28].copy(), np.zeros(2))
-    assert y0.tolist() == [428.0 - 29.0, 6296.0 - 667.0]
+    assert y0.tolist() == [float(v) for v in g["aprod1_y_noglob"][0]]
     x0 = oracle.aprod2(L0, a, idx, np.array([1.0, 2.0]), np.zeros(28))
-    assert x0[26] == 236.0 and x0.shape == (28,)
+    assert x0.shape == (28,)
+    for j, v in g["aprod2_x_noglob"]:
+        assert x0[j] == float(v)
 
 
 def test_col_map_matches_independent_map():
