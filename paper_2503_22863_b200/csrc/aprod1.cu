@@ -133,6 +133,8 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   SmemPlan p;
   p.stages = t.stages > 0 ? t.stages : 2;
   p.gather_smem = p.acc_smem = p.ins_tab = false;
+  p.tab_shift = 0;
+  p.acc_part = 0;
   const size_t table = ((size_t)s.I * 8 + 15) & ~(size_t)15;
   const bool want_acc = (what & PLAN_APROD2) && t.acc_smem, want_gather = (what & PLAN_APROD1) && t.gather_smem;
   const size_t want = (want_acc ? table : 0) + (want_gather ? table : 0);
@@ -147,8 +149,20 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
   if (want_acc && table <= left) { p.acc_smem = true; left -= table; }
   if (want_gather && table <= left) { p.gather_smem = true; left -= table; }
   // otherwise the aprod 2 side reduces into die-local chunked copies in L2: room for this CTA's chunk table
-  const size_t tab = ((size_t)((s.I + INS_CHUNK - 1) / INS_CHUNK) * sizeof(double*) + 15) & ~(size_t)15;
-  if ((what & PLAN_APROD2) && !p.acc_smem && tab <= left) { p.ins_tab = true; left -= tab; }
+  // (32 copies, one per bank, when they fit: 15 KB at C4; else one copy)
+  const size_t tab = ((size_t)((s.I + INS_CHUNK - 1) / INS_CHUNK) * sizeof(uint32_t) + 15) & ~(size_t)15;
+  if ((what & PLAN_APROD2) && !p.acc_smem) {
+    if (t.tab_private && 32 * tab <= left) { p.ins_tab = true; p.tab_shift = 5; left -= 32 * tab; }
+    else if (tab <= left) { p.ins_tab = true; left -= tab; }
+    const int want_part = what == PLAN_FUSED ? t.acc_part_fused : t.acc_part;
+    if (p.ins_tab && want_part) {
+      size_t ent = left / 8 & ~(size_t)1;
+      if (want_part > 0 && ent > (size_t)want_part) ent = (size_t)want_part & ~(size_t)1;
+      if ((int64_t)ent > s.I) ent = (size_t)s.I;
+      p.acc_part = (int)ent;
+      left -= ((ent + 1) & ~(size_t)1) * 8;
+    }
+  }
   p.bytes = SMEM_BUDGET - left;
   return p;
 }

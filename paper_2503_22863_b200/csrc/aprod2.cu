@@ -9,7 +9,7 @@ namespace gsr {
 template <bool ASMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
-             double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab,
+             double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
              const double* __restrict__ yscale, const int* done, int square) {
   if (done && *done) return;
   extern __shared__ char smem_raw[];
@@ -18,19 +18,16 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
-  double** tab_s = reinterpret_cast<double**>(acc_s);   // (only one of the two is in use)
+  uint32_t* tab_s = reinterpret_cast<uint32_t*>(acc_s + (ASMEM ? 0 : ((acc_part + 1) & ~1)));
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
-  if (ASMEM) {
-    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
-    __syncthreads();
-  } else if (use_tab) {
-    load_ins_tab(tab_s, ia);
-    __syncthreads();
-  }
-  ScatterCtx sc{x, gatt_il, x + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr};
+  const int64_t n_acc = ASMEM ? s.I : acc_part;   // accumulators privatised in shared memory: all, or the leading columns
+  for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
+  if (!ASMEM && use_tab) load_ins_tab(tab_s, ia, tab_shift);
+  if (n_acc || use_tab) __syncthreads();
+  ScatterCtx sc{x, gatt_il, x + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr, ia.base, tab_shift, (1 << tab_shift) - 1, acc_part};
   const AttLane al(lane);
   const double ys = yscale ? *yscale : 1.0;
   double gacc = 0.0;
@@ -60,13 +57,13 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     __syncwarp();
     att_scatter(tile, al, ts, gatt_il);
     astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x, square != 0);
-    gacc += scatter_rest<ASMEM>(row, valid, yv, sc);
+    gacc += scatter_rest<ASMEM>(row, lane, valid, yv, sc);
     ring.release(lane);
   }
-  if (ASMEM) {
+  if (n_acc) {
     __syncthreads();
     double* xins = x + s.oI;
-    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) {
+    for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) {
       const double v = acc_s[i];
       if (v != 0.0) atomicAdd(xins + i, v);
     }
@@ -167,7 +164,7 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
     InstrAcc ia = sd.ins;
     if (!t.die_local) ia.two_dies = false;
     k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc, ia,
-                                            use_copies ? 1 : 0, yscale, done, square);
+                                            use_copies ? 1 : 0, p.tab_shift, use_copies ? p.acc_part : 0, yscale, done, square);
     ++*launches;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

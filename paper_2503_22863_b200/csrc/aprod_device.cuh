@@ -34,6 +34,11 @@ __device__ __forceinline__ void red_add(double* p, double v) {
   asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+// the same, predicated on a >= b (no branch: keeps a run of reductions back to back in the instruction stream)
+__device__ __forceinline__ void red_add_if_ge(double* p, double v, int a, int b) {
+  asm volatile("{\n.reg .pred q;\nsetp.ge.s32 q, %2, %3;\n@q red.global.add.f64 [%0], %1;\n}" ::"l"(p), "d"(v), "r"(a), "r"(b) : "memory");
+}
+
 // What a kernel needs to gather from x (aprod 1 side).
 struct GatherCtx {
   const double* x;          // the n-vector being multiplied (astro block at x, 5 per star)
@@ -186,7 +191,11 @@ struct ScatterCtx {
   double* gatt_il;  // attitude accumulator, interleaved layout, 3K doubles
   double* xins;     // instrumental accumulator in global memory when neither of the next two is used: x + oI
   double* acc_s;    // shared-memory instrumental accumulator, or nullptr
-  double* const* ins_tab;   // shared-memory table of this CTA's die-local 4 KB accumulator chunks, or nullptr
+  const uint32_t* ins_tab;  // shared-memory table of this CTA's die-local 4 KB accumulator chunks, or nullptr:
+                            //   chunk c of the slice starts at ins_base + ins_tab[(c << tab_shift) | (lane & tab_mask)] doubles
+  double* ins_base;
+  int tab_shift, tab_mask;  // 5, 31: every lane reads its own bank (32 copies of the table, no bank conflicts); 0, 0: one copy
+  int acc_part;             // with ins_tab: columns [0, acc_part) are accumulated in acc_s instead (whatever shared memory is left)
 };
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -241,7 +250,7 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
 //  (Shared memory has no native fp64 add: atomicAdd is an LDS / DADD / ATOMS.CAST.SPIN loop.  Running the
 //  six chains of a row side by side with plain atomicCAS was measured SLOWER: aprod 2 at C2 0.72 vs 0.52 ms.)
 template <bool INSTR_SMEM>
-__device__ __forceinline__ double scatter_rest(const RowRegs& r, bool valid, double yv, const ScatterCtx& c) {
+__device__ __forceinline__ double scatter_rest(const RowRegs& r, int lane, bool valid, double yv, const ScatterCtx& c) {
   double gl = 0.0;
   if (valid) {
     const int col[6] = {r.i0.z, r.i0.w, r.i1.x, r.i1.y, r.i1.z, r.i1.w};
@@ -249,8 +258,21 @@ __device__ __forceinline__ double scatter_rest(const RowRegs& r, bool valid, dou
 #pragma unroll
     for (int q = 0; q < 6; q++) inc[q] = r.a[17 + q] * yv;
     if (!INSTR_SMEM && c.ins_tab) {
+      // what bounds the pass at C4 is L2 requests (an fp64 reduction costs ~1.65 of them), and shared-memory work
+      // runs in their shadow: every column that still fits shared memory is accumulated there.  The six L2
+      // reductions stay back to back as predicated instructions (a branch per slot serialised them: +15 %).
+      const int lsel = lane & c.tab_mask;
+      double* dst[6];
 #pragma unroll
-      for (int q = 0; q < 6; q++) red_add(c.ins_tab[col[q] >> INS_CHUNK_SHIFT] + (col[q] & (INS_CHUNK - 1)), inc[q]);
+      for (int q = 0; q < 6; q++)
+        dst[q] = c.ins_base + c.ins_tab[((col[q] >> INS_CHUNK_SHIFT) << c.tab_shift) | lsel] + (col[q] & (INS_CHUNK - 1));
+#pragma unroll
+      for (int q = 0; q < 6; q++) red_add_if_ge(dst[q], inc[q], col[q], c.acc_part);
+      if (c.acc_part) {
+#pragma unroll
+        for (int q = 0; q < 6; q++)
+          if (col[q] < c.acc_part) atomicAdd(c.acc_s + col[q], inc[q]);
+      }
     } else {
       if (INSTR_SMEM) {
 #pragma unroll
@@ -271,6 +293,8 @@ struct SmemPlan {
   bool gather_smem;   // instrumental slice of x staged in shared memory (aprod 1 side)
   bool acc_smem;      // instrumental accumulators privatised in shared memory (aprod 2 side)
   bool ins_tab;       // else: room reserved for the table of die-local accumulator chunks (InstrAcc)
+  int tab_shift;      // 5: the table is replicated 32 times, one copy per bank (LDS without bank conflicts); 0: one copy
+  int acc_part;       // with ins_tab: leading columns whose accumulators are privatised in the shared memory left over
   size_t bytes;       // dynamic shared memory to request
 };
 enum { PLAN_APROD1 = 1, PLAN_APROD2 = 2, PLAN_FUSED = 3 };
@@ -278,13 +302,16 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what);
 
 // This CTA's set of die-local accumulator chunks -> shared memory (n_chunks pointers).  Call before a
 // __syncthreads().  The set is chosen by the die of the SM the CTA runs on.
-__device__ __forceinline__ void load_ins_tab(double** tab_s, const InstrAcc& ia) {
+// Entry (c << tab_shift) + j, j < 2^tab_shift, is the offset (in doubles, from ia.base) of chunk c: with tab_shift = 5
+// lane l reads word 32 c + l, i.e. always its own bank (a single shared copy cost 5.5 wavefronts per LDS at C4).
+__device__ __forceinline__ void load_ins_tab(uint32_t* tab_s, const InstrAcc& ia, int tab_shift) {
   unsigned smid;
   asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
   int die = smid < (unsigned)SMID_SLOTS ? ia.sm_die[smid] : 0;
   if (die < 0 || !ia.two_dies) die = 0;
   const int set = die * ia.copies_per_die + (int)(blockIdx.x % (unsigned)ia.copies_per_die);
-  for (int i = threadIdx.x; i < ia.n_chunks; i += blockDim.x) tab_s[i] = ia.chunk_tab[(size_t)set * ia.n_chunks + i];
+  for (int i = threadIdx.x; i < (ia.n_chunks << tab_shift); i += blockDim.x)
+    tab_s[i] = (uint32_t)(ia.chunk_tab[(size_t)set * ia.n_chunks + (i >> tab_shift)] - ia.base);
 }
 
 __device__ __forceinline__ char* smem_align128(char* p) { return p + ((128u - (smem_u32(p) & 127u)) & 127u); }

@@ -206,6 +206,7 @@ static int build_instr_copies(gsr_system* s) {
     }
   e = cudaMemcpy(ia.chunk_tab, tab.data(), (size_t)need * sizeof(double*), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpy chunk table");
+  ia.base = base;
   ia.copies_per_die = (int)cpd;
   ia.n_chunks = (int)n_chunks;
   ia.two_dies = two != 0;
@@ -446,7 +447,7 @@ struct IterGraph {
   int64_t n_iters = 0, itnlim = 0, launches = 0, n_cov = 0;
   double atol = 0, btol = 0, conlim = 0;
   int fused = 0, warps = 0, stages = 0, acc_smem = 0, gather_smem = 0, die_local = 0, instr_copies = 0, ctas = 0;
-  int a1v = 0, a2v = 0;
+  int a1v = 0, a2v = 0, tabp = 0, accp = 0, accpf = 0;
   bool precond = false, var = false, cov = false;
   const void *j1 = nullptr, *j2 = nullptr, *covp = nullptr;
 };
@@ -454,7 +455,7 @@ static bool same_key(const IterGraph& a, const IterGraph& b) {
   return a.n_iters == b.n_iters && a.itnlim == b.itnlim && a.atol == b.atol && a.btol == b.btol && a.conlim == b.conlim &&
          a.fused == b.fused && a.warps == b.warps && a.stages == b.stages && a.acc_smem == b.acc_smem &&
          a.gather_smem == b.gather_smem && a.die_local == b.die_local && a.instr_copies == b.instr_copies &&
-         a.ctas == b.ctas && a.a1v == b.a1v && a.a2v == b.a2v && a.precond == b.precond && a.var == b.var &&
+         a.ctas == b.ctas && a.a1v == b.a1v && a.a2v == b.a2v && a.tabp == b.tabp && a.accp == b.accp && a.accpf == b.accpf && a.precond == b.precond && a.var == b.var &&
          a.cov == b.cov && a.n_cov == b.n_cov && a.j1 == b.j1 && a.j2 == b.j2 && a.covp == b.covp;
 }
 
@@ -480,7 +481,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
   key.n_iters = n_iters; key.itnlim = itnlim; key.atol = atol; key.btol = btol; key.conlim = conlim;
   key.fused = s->tune.fused; key.warps = s->tune.warps; key.stages = s->tune.stages; key.acc_smem = s->tune.acc_smem;
   key.gather_smem = s->tune.gather_smem; key.die_local = s->tune.die_local; key.instr_copies = s->tune.instr_copies;
-  key.ctas = s->tune.ctas_per_sm; key.a1v = s->tune.aprod1_variant; key.a2v = s->tune.aprod2_variant;
+  key.ctas = s->tune.ctas_per_sm; key.a1v = s->tune.aprod1_variant; key.a2v = s->tune.aprod2_variant; key.tabp = s->tune.tab_private; key.accp = s->tune.acc_part; key.accpf = s->tune.acc_part_fused;
   key.precond = s->opt_precond; key.var = s->opt_var; key.cov = s->opt_cov; key.n_cov = s->n_cov;
   key.j1 = s->cov_j1; key.j2 = s->cov_j2; key.covp = s->cov;
   IterGraph* g = s->iter_graph;
@@ -769,6 +770,9 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "die_local")) s->tune.die_local = (int)value;
   else if (!strcmp(name, "graph")) s->tune.graph = (int)value;
   else if (!strcmp(name, "gather_smem")) s->tune.gather_smem = (int)value;
+  else if (!strcmp(name, "tab_private")) s->tune.tab_private = (int)value;
+  else if (!strcmp(name, "acc_part")) s->tune.acc_part = (int)value;
+  else if (!strcmp(name, "acc_part_fused")) s->tune.acc_part_fused = (int)value;
   else if (!strcmp(name, "fused")) s->tune.fused = (int)value;
   else if (!strcmp(name, "check_every")) s->tune.check_every = (int)value;
   else return GSR_EINVAL;

@@ -47,6 +47,14 @@ struct Tuning {
   int acc_smem = 1;        // instrumental accumulators: 1 = privatised in shared memory when they fit, 0 = always L2 copies
   int die_local = 1;       // L2 instrumental accumulators: 1 = each CTA reduces into a copy homed on its own die, 0 = die-0 copies for all (control)
   int gather_smem = 1;     // instrumental slice of x: 1 = staged in shared memory when it fits, 0 = L1/L2 gathers
+  // L2 instrumental accumulators: leading columns privatised in whatever shared memory is left (-1 = all that fit,
+  // 0 = none, n = at most n).  Measured at the C4 shape (2e7 rows, profiles/r02_summary.md): standalone aprod 2
+  // 1.363 -> 1.222 ms with 6,000 of the 60,000 columns in shared memory; the fused pass keeps it off until measured
+  // in its predicated form (the first, branchy form cost it +15 %).
+  int acc_part = -1;       // standalone aprod 2
+  int acc_part_fused = 0;  // fused LSQR pass
+  int tab_private = 0;     // die-local chunk table: 1 = one copy per shared-memory bank (no LDS bank conflicts; measured -0.4 %:
+                           // shared-memory wavefronts are not what bounds the pass), 0 = one copy (leaves 15 KB to acc_part)
 };
 
 // Replicated instrumental accumulators for systems whose slice does not fit shared memory.
@@ -63,6 +71,7 @@ struct InstrAcc {
   double** chunk_tab = nullptr;  // device: [n_sets][n_chunks] chunk pointers; set = die * copies_per_die + copy
   int* sm_die = nullptr;         // device: [SMID_SLOTS] die (0 / 1) of an SM id
   void* pool = nullptr;          // device: the chunk pool (zero between calls)
+  double* base = nullptr;        // first 4 KB-aligned chunk of the pool (chunk pointers are base + 512 * index)
   int copies_per_die = 0, n_chunks = 0, n_sets = 0;   // n_sets = 2 * copies_per_die (copies_per_die if one die was seen)
   bool two_dies = false;
 };

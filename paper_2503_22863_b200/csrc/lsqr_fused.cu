@@ -16,7 +16,7 @@ namespace gsr {
 template <bool GSMEM, bool ASMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
-             double* __restrict__ uh, double* __restrict__ g, InstrAcc ia, int use_tab,
+             double* __restrict__ uh, double* __restrict__ g, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
              const double* __restrict__ c0p, double* usq, int* done) {
   {
     const int d = *done;
@@ -31,21 +31,21 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
-  double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : 0);
-  double** tab_s = reinterpret_cast<double**>(xi_s + (GSMEM ? ((s.I + 1) & ~1ll) : 0));
+  double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : ((acc_part + 1) & ~1));
+  uint32_t* tab_s = reinterpret_cast<uint32_t*>(xi_s + (GSMEM ? ((s.I + 1) & ~1ll) : 0));
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
-  if (ASMEM)
-    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) acc_s[i] = 0.0;
+  const int64_t n_acc = ASMEM ? s.I : acc_part;   // accumulators privatised in shared memory: all, or the leading columns
+  for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
   if (GSMEM)
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(v + s.oI + i);
-  if (!ASMEM && use_tab) load_ins_tab(tab_s, ia);
-  if (ASMEM || GSMEM || use_tab) __syncthreads();
+  if (!ASMEM && use_tab) load_ins_tab(tab_s, ia, tab_shift);
+  if (n_acc || GSMEM || use_tab) __syncthreads();
   const double* att_il = v + s.oA;
   GatherCtx gc{v, att_il, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
-  ScatterCtx sc{g, g + s.oA, g + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr};
+  ScatterCtx sc{g, g + s.oA, g + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr, ia.base, tab_shift, (1 << tab_shift) - 1, acc_part};
   const AttLane al(lane);
   const double c0 = *c0p;
   double sq = 0.0, gacc = 0.0;
@@ -81,13 +81,13 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     __syncwarp();
     att_scatter(tile, al, ts, sc.gatt_il);
     astro_scatter(tile, lane, nvalid, valid, row, out, sc.x);
-    gacc += scatter_rest<ASMEM>(row, valid, out, sc);
+    gacc += scatter_rest<ASMEM>(row, lane, valid, out, sc);
     ring.release(lane);
   }
-  if (ASMEM) {
+  if (n_acc) {
     __syncthreads();
     double* gins = g + s.oI;
-    for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) {
+    for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) {
       const double a = acc_s[i];
       if (a != 0.0) atomicAdd(gins + i, a);
     }
@@ -110,7 +110,7 @@ cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning
   if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
   const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
   const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
-  void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, InstrAcc, int, const double*, double*, int*);
+  void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, InstrAcc, int, int, int, const double*, double*, int*);
   if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true> : k_lsqr_fused<true, false>;
   else k = p.acc_smem ? k_lsqr_fused<false, true> : k_lsqr_fused<false, false>;
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
@@ -118,7 +118,7 @@ cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning
   ++*launches;
   InstrAcc ia = sd.ins;
   if (!t.die_local) ia.two_dies = false;
-  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, ia, use_copies ? 1 : 0, c0, usq, done);
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, ia, use_copies ? 1 : 0, p.tab_shift, use_copies ? p.acc_part : 0, c0, usq, done);
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (use_copies) return launch_fold_instr(s, sd, g, done, st, launches);
