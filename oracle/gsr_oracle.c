@@ -107,12 +107,22 @@ void orc_aprod1_abs(const orc_layout *L, int64_t nrows, const double *a, const i
 /* the steps either side of the LSQR loop in the paper's solver (PAPER.md:56,
  * 61, 63: "preconditioned" system, variances of the solution).  The paper gives no formulas; the
  * reading taken (R7) is diagonal column scaling by the column 2-norms.
- * nrm2sq[j] = sum_r a[r][k]^2 over the (r,k) with col(r,k) = j : squared 2-norm of column j. */
+ * nrm2sq[j] += sum_r (A[r][j])^2, where A[r][j] = sum of the a[r][k] with col(r,k) = j : the squared 2-norm of
+ * column j of A as an operator.  A column can repeat inside a row (instrumental slots): the
+ * coefficients of equal columns are summed first, in slot order, and the sum is squared once. */
 void orc_colnorm2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, double *nrm2sq) {
   for (int64_t r = 0; r < nrows; r++)
     for (int k = 0; k < NSLOT; k++) {
       int64_t c = orc_col(L, idx + r * NIDX, k);
-      if (c >= 0) nrm2sq[c] += a[r * NSLOT + k] * a[r * NSLOT + k];
+      if (c < 0) continue;
+      int seen = 0;                         /* an earlier slot of this row already carried column c */
+      for (int k0 = 0; k0 < k; k0++)
+        if (orc_col(L, idx + r * NIDX, k0) == c) seen = 1;
+      if (seen) continue;
+      double arj = a[r * NSLOT + k];        /* A[r][c]: this slot and every later slot on the same column */
+      for (int k1 = k + 1; k1 < NSLOT; k1++)
+        if (orc_col(L, idx + r * NIDX, k1) == c) arj += a[r * NSLOT + k1];
+      nrm2sq[c] += arj * arj;
     }
 }
 /* a_out[r][k] = a[r][k] * s[col(r,k)] : the matrix A diag(s), same index records. */

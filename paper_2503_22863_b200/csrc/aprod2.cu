@@ -47,6 +47,18 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     RowRegs row;
     load_row(tile, lane, valid, row);
     if (square) {
+      // squared column norms of A as an operator: a column that repeats inside a row (instrumental slots only)
+      // contributes (sum of its coefficients)^2 once -- summed in slot order into the first of its slots
+      const int col[6] = {row.i0.z, row.i0.w, row.i1.x, row.i1.y, row.i1.z, row.i1.w};
+      bool dup[6] = {false, false, false, false, false, false};
+#pragma unroll
+      for (int q = 0; q < 6; q++) {
+        double sum = row.a[17 + q];
+#pragma unroll
+        for (int p = q + 1; p < 6; p++)
+          if (!dup[q] && col[p] == col[q]) { sum += row.a[17 + p]; dup[p] = true; }
+        row.a[17 + q] = dup[q] ? 0.0 : sum;
+      }
 #pragma unroll
       for (int k = 0; k < NSLOT; k++) row.a[k] *= row.a[k];
     }

@@ -42,6 +42,9 @@ def badly_scaled(shape, seed_scale=3):
                          ids=["tiny-noglob", "C1", "C5-small"])
 def test_colnorms(shape):
     a, idx = badly_scaled(shape)
+    # repeated instrumental columns inside a row (two pairs, and a triple): ||A e_j||_2 sums them before squaring
+    idx[::4, 2:8] = np.array([1, 1, 3, 0, 5, 3], dtype=np.int32)
+    idx[1::8, 2:8] = np.array([2, 4, 2, 6, 2, 0], dtype=np.int32)
     ref = oracle.colnorms(oracle.layout_of(shape), a, idx)
     with make(shape, a, idx) as s:
         out = torch.empty(s.n_unknowns, dtype=torch.float64, device=DEV)

@@ -389,14 +389,13 @@ def test_colnorms_match_dense_columns():
         D = dense_matrix(shape, a, idx)
         got = oracle.colnorms(oracle.layout_of(shape), a, idx)
         # a repeated column inside one row: the dense matrix holds the SUM of the two coefficients, the
-        # column norm of A as an operator; the oracle must agree with that, not with sum of squares
-        rows_dup = np.arange(0, a.shape[0], 4)
+        # column norm of A as an operator; the oracle must agree with that, not with the sum of squares
         ref = np.linalg.norm(D, axis=0)
         dup_cols = shape.off_instr + np.array([1, 3])
-        mask = np.ones(shape.n_unknowns, dtype=bool)
-        mask[dup_cols] = False
-        assert np.allclose(got[mask], ref[mask], rtol=1e-14, atol=0)
-        assert np.all(got[ref == 0.0] == 0.0) and len(rows_dup) > 0
+        assert np.allclose(got, ref, rtol=1e-14, atol=0)
+        sumsq = np.sqrt(np.sum(a[:, 17:23] ** 2 * (idx[:, 2:8] == 1), axis=0).sum())   # what a per-slot sum would give
+        assert abs(sumsq - ref[dup_cols[0]]) > 1e-3 * ref[dup_cols[0]]                  # (the case does discriminate)
+        assert np.all(got[ref == 0.0] == 0.0)
 
 
 def test_scale_columns_is_right_multiplication_by_a_diagonal():
