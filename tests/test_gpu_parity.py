@@ -22,6 +22,7 @@ import paper_2503_22863_b200 as gsr  # noqa: E402
 from gaia_synth import device as gdev  # noqa: E402
 from gaia_synth import host  # noqa: E402
 from gaia_synth.configs import C1, C2, C3, C5, SystemShape  # noqa: E402
+from gpu_helpers import gpu_state, oracle_state_from, replay_one_step  # noqa: E402,F401
 from helpers import nonempty_columns, rhs, tiny_shape  # noqa: E402
 
 DEV = "cuda"
@@ -230,42 +231,6 @@ def test_empty_system_and_errors():
 
 
 # ------------------------------------------------------------------ LSQR
-def gpu_state(s, m, n):
-    u = torch.empty(m, dtype=torch.float64, device=DEV)
-    v, w, x = (torch.empty(n, dtype=torch.float64, device=DEV) for _ in range(3))
-    sc = s.lsqr_state(u, v, w, x)
-    return {"u": u.cpu().numpy(), "v": v.cpu().numpy(), "w": w.cpu().numpy(), "x": x.cpu().numpy()}, sc
-
-
-def oracle_state_from(vecs, sc, m, n):
-    st = oracle.LsqrState(m, n)
-    for k in ("u", "v", "w", "x"):
-        getattr(st, k)[:] = vecs[k]
-    for k, val in sc.items():
-        setattr(st, k, val)
-    return st
-
-
-def replay_one_step(shape, a, idx, s, tol_vec=1e-11, tol_sc=1e-10, threads=1):
-    """GPU state at k -> one ORACLE iteration -> must equal the GPU state at k+1."""
-    L = oracle.layout_of(shape)
-    m, n = a.shape[0], shape.n_unknowns
-    vecs, sc = gpu_state(s, m, n)
-    st = oracle_state_from(vecs, sc, m, n)
-    oracle.lsqr_step(L, a, idx, st, threads=threads)
-    s.lsqr_iterate(1)
-    vecs1, sc1 = gpu_state(s, m, n)
-    assert sc1["itn"] == st.itn
-    for k in ("u", "v", "w", "x"):
-        ref = getattr(st, k)
-        e = np.linalg.norm(vecs1[k] - ref) / np.linalg.norm(ref)
-        assert e <= tol_vec, f"one-step replay at itn {st.itn}: vector {k} off by {e:.3e}"
-    for k in ("alpha", "beta", "rhobar", "phibar", "rnorm", "arnorm", "anorm", "acond", "ddnorm", "xnorm",
-              "xxnorm", "z", "cs2", "sn2", "bnorm"):
-        ref = getattr(st, k)
-        assert abs(sc1[k] - ref) <= tol_sc * abs(ref) + 1e-300, f"one-step replay at itn {st.itn}: {k} {sc1[k]} vs {ref}"
-
-
 def test_lsqr_c1_to_convergence():
     a, idx = host.make_rows(C1)
     L = oracle.layout_of(C1)
