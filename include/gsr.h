@@ -34,6 +34,16 @@
  * ERRORS.  Every int-returning call returns GSR_OK (0) or a negative code; nothing is printed,
  * nothing throws, nothing exits.  gsr_strerror() names a code.
  *
+ * THREADS AND STREAMS.  A gsr_system is NOT re-entrant: every call on one system shares its scratch
+ * (interleaved attitude buffers, the replicated instrumental accumulators, which are assumed zero
+ * between calls, the LSQR work vectors and the single set of device-resident scalars).  All calls on
+ * one system must therefore be issued on ONE stream, or be ordered externally (events) so that no two
+ * of them overlap; two gsr_aprod2 calls, or gsr_aprod2 / gsr_colnorms next to gsr_lsqr_iterate, running
+ * concurrently on one system corrupt each other's results silently.  Different systems may run
+ * concurrently on different streams from ONE host thread; the library is not thread-safe across
+ * systems either (kernel attributes such as the dynamic shared-memory limit are process-global and are
+ * set at launch time), so calls from several host threads must be serialised by the caller.
+ *
  * DETERMINISM.  aprod2 uses fp64 reductions at L2 (red.global.add.f64) for the attitude block;
  * the order of those additions varies run to run, so results are reproducible to rounding
  * (normwise ~1e-15), not bit for bit.  aprod1 is bit-reproducible.
@@ -62,8 +72,11 @@ typedef struct {
   int64_t n_knots; /* K : attitude block = 3*K columns, axis offset K; K >= 4         */
   int64_t n_instr; /* I : instrumental block; I >= 1                                  */
   int32_t n_glob;  /* G : 0 or 1 (the paper's tests use 0)              */
-  int32_t flags;   /* reserved, must be 0                                             */
+  int32_t flags;   /* 0, or GSR_LAYOUT_TRUSTED: the caller guarantees that every index record
+                      is in range and that rows are sorted by star; gsr_create then skips its
+                      device-side validation pass (4 ms at 5e8 rows).  Other bits: GSR_EINVAL */
 } gsr_layout;
+#define GSR_LAYOUT_TRUSTED 1
 
 typedef struct {
   int32_t istop; /* Paige-Saunders stop code 0..7 (not an error)                      */
@@ -176,12 +189,17 @@ int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_
  *                    (aprod 1 + aprod 2 of one iteration in one sweep over A) (host out-pointers).
  * gsr_set_option   : tuning knobs (measured in profiles/r01_summary.md section 3);
  *                    unknown names -> GSR_EINVAL.  Names (value 0 = default of the planner unless stated):
- *                      warps, stages     warps per CTA (<= 12) and TMA ring depth per warp of the tile kernels
+ *                      warps, stages     warps per CTA (<= 12; planner default 12, down to 8 when that lets the instrumental
+ *                                        tables fit shared memory) and TMA ring depth per warp (default 2) of the tile kernels
  *                      ctas_per_sm       CTAs per SM (default 1)
  *                      acc_smem          1 (default) privatise the instrumental accumulators in shared memory
  *                                        when they fit, 0 always reduce into the L2-resident copies
  *                      die_local         1 (default) L2-resident instrumental accumulators: every CTA reduces into a copy whose
  *                                        4 KB chunks are homed on the L2 of its own die (probed at gsr_create), 0 control
+ *                      acc_part, acc_part_fused   when the accumulators live in L2: how many leading instrumental columns are
+ *                                        accumulated in left-over shared memory instead (-1 all that fit, 0 none; standalone
+ *                                        aprod 2 default -1, fused LSQR pass default 0)
+ *                      tab_private       1: the table of die-local chunks is replicated once per shared-memory bank, 0 (default) one copy
  *                      gather_smem       1 (default) stage the instrumental slice of x in shared memory when it fits
  *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x
  *                      fused             1 (default) one pass over A per LSQR iteration, 0 aprod 1 then aprod 2

@@ -51,6 +51,7 @@ class LsqrResult:
 
 
 GSR_PRECOND_COLNORM = 1
+GSR_LAYOUT_TRUSTED = 1
 
 _lib = None
 
@@ -137,10 +138,11 @@ class GsrSystem:
 
     values: CUDA float64 [M,24]; indices: CUDA int32 [M,8] -- borrowed, kept alive by this object."""
 
-    def __init__(self, n_stars, n_knots, n_instr, n_glob, values, indices):
+    def __init__(self, n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False):
         import torch
         m = int(values.shape[0]) if values is not None else 0
-        self.layout = _Layout(m, int(n_stars), int(n_knots), int(n_instr), int(n_glob), 0)
+        self.layout = _Layout(m, int(n_stars), int(n_knots), int(n_instr), int(n_glob),
+                              GSR_LAYOUT_TRUSTED if trusted else 0)
         self._values, self._indices = values, indices
         self._h = _vp()
         vp = _dev_ptr(values, torch.float64, m * 24, "values")
@@ -270,8 +272,9 @@ class GsrSystem:
 
 
 # ---- free functions with the C names ----------------------------------------------------------
-def gsr_create(n_stars, n_knots, n_instr, n_glob, values, indices) -> GsrSystem:
-    return GsrSystem(n_stars, n_knots, n_instr, n_glob, values, indices)
+def gsr_create(n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False) -> GsrSystem:
+    """trusted=True sets GSR_LAYOUT_TRUSTED (the caller vouches for the index records; no validation pass)."""
+    return GsrSystem(n_stars, n_knots, n_instr, n_glob, values, indices, trusted)
 
 
 def gsr_destroy(sys: GsrSystem):
@@ -298,8 +301,10 @@ def _host_ptr(a, np_dtype, numel, name):
         if isinstance(a, torch.Tensor):
             if a.is_cuda:
                 raise TypeError(f"{name}: gsr_lsqr_host takes HOST buffers")
-            if not a.is_contiguous() or a.numel() != numel:
-                raise ValueError(f"{name}: need a contiguous host buffer of {numel} elements")
+            want = {np.dtype(np.float64): torch.float64, np.dtype(np.int32): torch.int32}[np.dtype(np_dtype)]
+            if a.dtype != want or not a.is_contiguous() or a.numel() != numel:
+                raise ValueError(f"{name}: need a contiguous {want} host buffer of {numel} elements, "
+                                 f"got {a.dtype} {tuple(a.shape)}")
             return a.data_ptr()
     except ImportError:
         pass

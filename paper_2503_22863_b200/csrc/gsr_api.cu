@@ -22,6 +22,20 @@ static int cuda_fail(cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call);    \
   } while (0)
 
+// cudaMalloc with the ABI's error mapping: an allocation failure is GSR_ENOMEM (and is not left pending).
+static int dev_alloc(void** p, size_t bytes, const char* what) {
+  cudaError_t e = cudaMalloc(p, bytes);
+  if (e == cudaSuccess) return GSR_OK;
+  *p = nullptr;
+  cudaGetLastError();
+  return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, what);
+}
+#define ALLOC(ptr, bytes)                                                        \
+  do {                                                                           \
+    int rc_ = dev_alloc(reinterpret_cast<void**>(&(ptr)), (bytes), #ptr);        \
+    if (rc_) return rc_;                                                         \
+  } while (0)
+
 struct EventPair {
   cudaEvent_t a, b;
   int which;
@@ -214,15 +228,20 @@ static int build_instr_copies(gsr_system* s) {
   return GSR_OK;
 }
 
+static int check_layout(const gsr_layout* L) {
+  if (!L) return GSR_EINVAL;
+  if (L->n_rows < 0 || L->n_stars < 1 || L->n_knots < 4 || L->n_instr < 1) return GSR_EINVAL;
+  if (L->n_glob != 0 && L->n_glob != 1) return GSR_EINVAL;
+  if (L->flags & ~GSR_LAYOUT_TRUSTED) return GSR_EINVAL;
+  if (L->n_stars > INT32_MAX || L->n_knots > INT32_MAX || L->n_instr > INT32_MAX) return GSR_EINVAL;
+  return GSR_OK;
+}
+
 extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* values,
                           const int32_t* indices, void* stream) {
   if (!out) return GSR_EINVAL;
   *out = nullptr;
-  if (!L) return GSR_EINVAL;
-  if (L->n_rows < 0 || L->n_stars < 1 || L->n_knots < 4 || L->n_instr < 1) return GSR_EINVAL;
-  if (L->n_glob != 0 && L->n_glob != 1) return GSR_EINVAL;
-  if (L->flags != 0) return GSR_EINVAL;
-  if (L->n_stars > INT32_MAX || L->n_knots > INT32_MAX || L->n_instr > INT32_MAX) return GSR_EINVAL;
+  if (check_layout(L)) return GSR_EINVAL;
   if (L->n_rows > 0 && (!values || !indices)) return GSR_EINVAL;
   if (!aligned(values, 32) || !aligned(indices, 32)) return GSR_EINVAL;
   int dev = 0;
@@ -236,19 +255,21 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
   v.vals = values; v.idx = indices;
   v.M = L->n_rows; v.S = L->n_stars; v.K = L->n_knots; v.I = L->n_instr; v.G = L->n_glob;
   v.oA = 5 * v.S; v.oI = v.oA + 3 * v.K; v.oG = v.oI + v.I; v.n = v.oG + v.G;
-  // device-side validation of every index record
-  int* flag = nullptr;
-  e = cudaMalloc(&flag, sizeof(int));
-  if (e != cudaSuccess) { delete s; return e == cudaErrorMemoryAllocation ? GSR_ENOMEM : cuda_fail(e, "cudaMalloc"); }
-  int h = 0;
-  cudaStream_t st = S(stream);
-  e = cudaMemsetAsync(flag, 0, sizeof(int), st);
-  if (e == cudaSuccess) e = launch_validate(v, flag, st, &s->launches);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(flag);
-  if (e != cudaSuccess) { delete s; return cuda_fail(e, "gsr_create validation"); }
-  if (h != 0) { delete s; return GSR_ELAYOUT; }
+  // device-side validation of every index record (skipped when the caller vouches for them)
+  if (!(L->flags & GSR_LAYOUT_TRUSTED)) {
+    int* flag = nullptr;
+    int rc = dev_alloc(reinterpret_cast<void**>(&flag), sizeof(int), "cudaMalloc flag");
+    if (rc) { delete s; return rc; }
+    int h = 0;
+    cudaStream_t st = S(stream);
+    e = cudaMemsetAsync(flag, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = launch_validate(v, flag, st, &s->launches);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(flag);
+    if (e != cudaSuccess) { delete s; return cuda_fail(e, "gsr_create validation"); }
+    if (h != 0) { delete s; return GSR_ELAYOUT; }
+  }
   // side structures: the row-tile tensor map, the interleaved attitude buffers, instrumental replicas
   if (v.M > 0) {
     int rc = make_row_tensor_map(&s->side.map, values, v.M);
@@ -354,8 +375,8 @@ static int ensure_workspace(gsr_system* s) {
 // D^-1 (internal layout): one pass over A for the squared column norms, then 1/sqrt with the empty-column guard.
 static int build_dinv(gsr_system* s, cudaStream_t st) {
   const size_t n = (size_t)s->v.n;
-  if (!s->dinv) CU(cudaMalloc(&s->dinv, n * sizeof(double)));
-  if (!s->vs) CU(cudaMalloc(&s->vs, n * sizeof(double)));
+  if (!s->dinv) ALLOC(s->dinv, n * sizeof(double));
+  if (!s->vs) ALLOC(s->vs, n * sizeof(double));
   CU(cudaMemsetAsync(s->dinv, 0, n * sizeof(double), st));
   CU(launch_aprod2(s->v, s->side, s->tune, s->num_sms, nullptr, s->dinv, true, nullptr, nullptr, st, &s->launches, 1));
   CU(lsqr_launch_colnorm_finish(s->dinv, s->v.n, 1, st, &s->launches));
@@ -377,7 +398,7 @@ static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool wan
   s->opt_precond = precond;
   s->opt_var = want_var;
   if (precond && (rc = build_dinv(s, S(stream)))) return rc;
-  if (want_var && !s->var) CU(cudaMalloc(&s->var, (size_t)s->v.n * sizeof(double)));
+  if (want_var && !s->var) ALLOC(s->var, (size_t)s->v.n * sizeof(double));
   s->opt_cov = s->opt_cov_next && s->n_cov > 0;
   if (s->opt_cov) CU(cudaMemsetAsync(s->cov, 0, (size_t)s->n_cov * sizeof(double), S(stream)));
   cudaStream_t st = S(stream);
@@ -468,15 +489,19 @@ static void free_iter_graph(gsr_system* s) {
   if (s->cap_stream) { cudaStreamDestroy(s->cap_stream); s->cap_stream = nullptr; }
 }
 
+// a batch of n_iters iterations is replayed as a CUDA graph (small, launch-bound systems only)
+static bool graph_path(const gsr_system* s, int64_t n_iters) {
+  const bool small = (double)s->v.M * 224.0 <= 256.0 * 1024 * 1024;
+  return s->tune.graph && !s->profile && n_iters >= 2 && small;
+}
+
 extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, double atol, double btol,
                                 double conlim, void* stream) {
   if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
   if (!s->lsqr_ready) return GSR_ESTATE;
   if (s->opt_precond && !s->tune.fused) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
   cudaStream_t st = S(stream);
-  const bool small = (double)s->v.M * 224.0 <= 256.0 * 1024 * 1024;
-  if (!s->tune.graph || s->profile || n_iters < 2 || !small)
-    return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
+  if (!graph_path(s, n_iters)) return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
   IterGraph key;
   key.n_iters = n_iters; key.itnlim = itnlim; key.atol = atol; key.btol = btol; key.conlim = conlim;
   key.fused = s->tune.fused; key.warps = s->tune.warps; key.stages = s->tune.stages; key.acc_smem = s->tune.acc_smem;
@@ -602,7 +627,7 @@ extern "C" int gsr_set_cov_pairs(gsr_system* s, const int64_t* j1, const int64_t
   cudaStream_t st = S(stream);
   int* bad = nullptr;
   int h = 0;
-  CU(cudaMalloc(&bad, sizeof(int)));
+  ALLOC(bad, sizeof(int));
   cudaError_t e = cudaMemsetAsync(bad, 0, sizeof(int), st);
   if (e == cudaSuccess) e = lsqr_launch_check_pairs(j1, j2, n_pairs, s->v.n, bad, st, &s->launches);
   if (e == cudaSuccess) e = cudaMemcpyAsync(&h, bad, sizeof(int), cudaMemcpyDeviceToHost, st);
@@ -648,7 +673,9 @@ static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int3
   int64_t issued = 0;
   while (!h.done && issued < itnlim) {
     int64_t batch = s->tune.check_every > 0 ? s->tune.check_every : 16;
-    if (batch > itnlim - issued) batch = itnlim - issued;
+    // On the graph path the batch size is baked into the cached graph, so the last batch stays whole: iterations past
+    // itnlim are no-ops on the device (k_step_scalars sets istop = 7 and the stop flag).  Eagerly, issue what is left.
+    if (batch > itnlim - issued && !graph_path(s, batch)) batch = itnlim - issued;
     if ((rc = gsr_lsqr_iterate(s, batch, itnlim, atol, btol, conlim, stream))) return rc;
     issued += batch;
     if ((rc = fetch_scalars(s, &h, st))) return rc;   // poll the device-side stop flag
@@ -669,7 +696,7 @@ static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int3
 extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, const int32_t* indices_host,
                              const double* b_host, double* x_host, int64_t itnlim, double atol, double btol,
                              double conlim, gsr_lsqr_result* res) {
-  if (!L || !x_host || !res || L->n_rows < 0) return GSR_EINVAL;
+  if (!x_host || !res || check_layout(L)) return GSR_EINVAL;   // (before any size is computed from the layout)
   if (L->n_rows > 0 && (!values_host || !indices_host || !b_host)) return GSR_EINVAL;
   const size_t M = (size_t)L->n_rows;
   const size_t n = (size_t)(5 * L->n_stars + 3 * L->n_knots + L->n_instr + L->n_glob);

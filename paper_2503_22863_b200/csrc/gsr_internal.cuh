@@ -38,8 +38,8 @@ struct Tuning {
   int aprod1_variant = 1;  // 1 = TMA-staged tiles (default), 0 = one thread per row (simple)
   int aprod2_variant = 1;  // 1 = TMA-staged tiles, split by parameter block (default), 0 = one thread per row
   int ctas_per_sm = 0;     // 0 = default of the variant
-  int warps = 0;           // warps per CTA of the TMA kernels (0 = default 8)
-  int stages = 0;          // ring depth per warp (0 = default 3)
+  int warps = 0;           // warps per CTA of the TMA kernels (0 = the planner's choice: 12, down to 8 if that lets the tables fit)
+  int stages = 0;          // ring depth per warp (0 = default 2)
   int check_every = 16;    // LSQR iterations between host polls of the stop flag
   int instr_copies = 1;    // replicate the instrumental accumulator in global memory when it cannot be privatised
   int fused = 1;           // LSQR: one fused pass over the matrix per iteration (lsqr_fused.cu)

@@ -49,9 +49,34 @@ def test_argument_validation_without_gpu(libgsr):
     assert libgsr.gsr_create(ct.byref(h), ct.byref(bad), None, None, None) == -1
     bad = _Layout(10, 1, 8, 6, 1, 0)                                   # null arrays with M > 0
     assert libgsr.gsr_create(ct.byref(h), ct.byref(bad), None, None, None) == -1
+    bad = _Layout(10, 1, 8, 6, 1, 2)                                   # unknown flag bit
+    assert libgsr.gsr_create(ct.byref(h), ct.byref(bad), None, None, None) == -1
     assert libgsr.gsr_aprod1(None, None, None, None) == -1
     assert libgsr.gsr_lsqr_iterate(None, 1, 1, 0.0, 0.0, 0.0, None) == -1
     libgsr.gsr_destroy(None)                                           # no-op
+
+
+def test_host_entry_validates_before_it_sizes_anything(libgsr):
+    """gsr_lsqr_host computes allocation sizes from the layout: a bad layout must be GSR_EINVAL, not GSR_ENOMEM,
+    and a host buffer of the wrong dtype must be refused by the binding (it would be read past its end)."""
+    import numpy as np
+    import torch
+    from paper_2503_22863_b200 import binding
+    from paper_2503_22863_b200.binding import _Layout, _Result
+    r = _Result()
+    x = np.zeros(64)
+    for bad in (_Layout(4, -3, 8, 6, 1, 0), _Layout(4, 1, 2, 6, 1, 0), _Layout(4, 1, 8, 0, 1, 0), _Layout(4, 1, 8, 6, 5, 0),
+                _Layout(-1, 1, 8, 6, 1, 0), _Layout(4, 1, 8, 6, 1, 4)):
+        rc = libgsr.gsr_lsqr_host(ct.byref(bad), x.ctypes.data, x.ctypes.data, x.ctypes.data, x.ctypes.data, 1, 0.0, 0.0,
+                                  0.0, ct.byref(r))
+        assert rc == -1
+    with pytest.raises(ValueError):      # float32 values of the right element count
+        binding._host_ptr(torch.zeros(4 * 24, dtype=torch.float32), np.float64, 4 * 24, "values")
+    with pytest.raises(ValueError):      # int64 indices
+        binding._host_ptr(torch.zeros(4 * 8, dtype=torch.int64), np.int32, 4 * 8, "indices")
+    with pytest.raises(ValueError):
+        binding._host_ptr(np.zeros(4 * 8, dtype=np.int64), np.int32, 4 * 8, "indices")
+    assert binding._host_ptr(torch.zeros(4 * 8, dtype=torch.int32), np.int32, 4 * 8, "indices") != 0
 
 
 def test_no_cpu_fallback():
