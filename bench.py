@@ -3,6 +3,11 @@
 vector work) and achieved HBM GB/s, on a synthetic Gaia-shaped system (BASELINE.json).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--impl reference]
+                    [--control uniform-starts] [--mode extras] [--option name=value ...]
+
+`--control uniform-starts` runs the same workload with uniform attitude starts (the control of C3's hot knots: same
+rows per star, same M); `--mode extras` times what sits either side of the loop (gsr_colnorms, gsr_lsqr_ex with
+preconditioning and variances, covariance pairs) instead of the iteration; `--option` passes gsr_set_option knobs.
 
 One "step" = one LSQR iteration = one pass of the whole hot path over the system.  The system is
 generated in HBM by the seeded generator before the timed region; the matrix (>= 2 GB) is far
@@ -42,6 +47,12 @@ def parse():
     ap.add_argument("--option", action="append", default=[], help="name=value passed to gsr_set_option")
     ap.add_argument("--stars", type=int, default=0,
                     help="profiling aid: same workload family with this many stars (K, I unchanged); 0 = the config's")
+    ap.add_argument("--control", default="none", choices=["none", "uniform-starts"],
+                    help="uniform-starts: the workload with uniform attitude starts instead of its hot-knot mixture")
+    ap.add_argument("--mode", default="iterate", choices=["iterate", "extras"],
+                    help="extras: time gsr_colnorms / gsr_lsqr_ex (preconditioned, variances) / covariance pairs")
+    ap.add_argument("--reps", type=int, default=20, help="repetitions of the single aprod 1 / aprod 2 timings")
+    ap.add_argument("--cov-pairs", type=int, action="append", default=[], help="--mode extras: pair counts to time")
     return ap.parse_args()
 
 
@@ -133,27 +144,41 @@ def measured_peak():
 
 
 def ncu_traffic(kernel, m):
-    """dram bytes per launch from the committed ncu --set full summary (profiles/r01_traffic.csv:
-    bytes per row of one captured launch), scaled by the rows of this workload; else None."""
+    """(dram bytes per launch, where the figure comes from).  profiles/r02_traffic.csv, when present, holds
+    dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full` capture of a launch together with the
+    rows of that launch; else profiles/r01_traffic.csv (C4 layout at 2e7 rows).  A capture of another size is
+    scaled by rows and says so.  (None, reason) when there is no capture for this kernel."""
     import csv
-    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    try:
-        with open(p) as f:
-            for row in csv.DictReader(f):
-                if row["kernel"] == kernel:
-                    return float(row["dram_bytes_per_row"]) * m
-    except Exception:
-        pass
-    return None
+    for name in ("r02_traffic.csv", "r01_traffic.csv"):
+        p = os.path.join(ROOT, "profiles", name)
+        try:
+            with open(p) as f:
+                for row in csv.DictReader(f):
+                    if row["kernel"] != kernel:
+                        continue
+                    per_row = float(row["dram_bytes_per_row"])
+                    rows = int(float(row.get("rows") or 20_000_000))
+                    src = f"profiles/{name}: ncu --set full capture of one launch at {rows} rows"
+                    if rows != m:
+                        src += f", {per_row:.1f} B/row scaled to {m} rows"
+                    return per_row * m, src
+        except Exception:
+            continue
+    return None, "no ncu capture committed for this kernel"
 
 
-def pick_workload(name, free_bytes):
+def pick_workload(name, free_bytes, control="none"):
+    from dataclasses import replace
     from gaia_synth.configs import CONFIGS
     if name != "auto":
-        return CONFIGS[name]
-    c4 = CONFIGS["C4"]
-    need = 5e8 * (192 + 32 + 8 + 8) + 5 * c4.n_unknowns * 8 + (4 << 30)
-    return c4 if free_bytes >= need else CONFIGS["C2"]
+        shape = CONFIGS[name]
+    else:
+        c4 = CONFIGS["C4"]
+        need = 5e8 * (192 + 32 + 8 + 8) + 5 * c4.n_unknowns * 8 + (4 << 30)
+        shape = c4 if free_bytes >= need else CONFIGS["C2"]
+    if control == "uniform-starts":
+        shape = replace(shape, hot_knots=False, name=shape.name + "[uniform attitude starts]")
+    return shape
 
 
 def shape_rows(shape):
@@ -162,9 +187,10 @@ def shape_rows(shape):
 
 
 # ------------------------------------------------------------------------------------ oracle timing
-def time_oracle(shape, m_full, a, idx, steps, warmup):
+def time_oracle(shape, m_full, a, idx, steps, warmup, budget_s=1e9):
     """ms per LSQR iteration of the CPU oracle (OpenMP, all cores) on a row sample [a, idx] of the
-    workload, extrapolated to m_full rows: t = t_rows * (m_full / sample) + t_vectors."""
+    workload, extrapolated to m_full rows: t = t_rows * (m_full / sample) + t_vectors.
+    Stops early (after at least one timed step) once budget_s seconds have gone into the loop."""
     import numpy as np
     import oracle
     from gaia_synth import host
@@ -176,6 +202,7 @@ def time_oracle(shape, m_full, a, idx, steps, warmup):
     x = host.test_vector(1, 1, n)
     y = np.zeros(ms)
     t_step, t_rows = [], []
+    t_begin = time.perf_counter()
     for it in range(warmup + steps):
         t0 = time.perf_counter()
         oracle.lsqr_step(L, a, idx, st, threads=th)
@@ -186,45 +213,72 @@ def time_oracle(shape, m_full, a, idx, steps, warmup):
         if it >= warmup:
             t_step.append(t1 - t0)
             t_rows.append(t2 - t1)
+            if t2 - t_begin > budget_s:
+                break
     step = sum(t_step) / len(t_step)
     rows = min(sum(t_rows) / len(t_rows), step)
     full = rows * (m_full / ms) + (step - rows)
-    return {"value": full * 1e3, "unit": "ms", "cores": th, "kind": "oracle",
-            "sample": f"first {ms} of {m_full} rows of {shape.name} (OpenMP oracle, {steps} LSQR iterations; "
+    return {"value": full * 1e3, "unit": "ms", "cores": th, "kind": "oracle", "steps_timed": len(t_step),
+            "sample": f"first {ms} of {m_full} rows of {shape.name} (OpenMP oracle, {len(t_step)} LSQR iterations timed; "
                       f"measured {step * 1e3:.1f} ms/iteration on the sample, row part scaled by {m_full / ms:.1f})"}
 
 
 def oracle_sample_rows(m_full, requested):
+    """Rows of the oracle's sample: the whole workload up to 1e8 rows ("time the first 1e8 rows (22 GB)"
+    when the host cannot hold C4), less if host memory is short."""
     if requested > 0:
         return min(requested, m_full)
-    return min(m_full, 4_000_000)
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        avail = 16 << 30
+    cap = int(max(avail * 0.4, 1 << 30) // 260)        # rows + the M-vectors of the oracle's LSQR state
+    return max(1, min(m_full, 100_000_000, cap))
 
 
 # ------------------------------------------------------------------------------------ reference arm
 def run_reference(args):
-    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload.  The sample rows come
+    from the device generator when a GPU is there (the numpy generator needs minutes for 1e8 rows), copied to the host."""
     rank, local_rank, world = dist_env()
     if rank != 0:
         return 0
     import oracle  # noqa: F401  (the one other place bench.py may execute oracle/)
     from gaia_synth import host
     from gaia_synth.configs import CONFIGS
+    cuda = False
     try:
         import torch
-        free = torch.cuda.mem_get_info()[0] if torch.cuda.is_available() else 0
+        cuda = torch.cuda.is_available()
+        free = torch.cuda.mem_get_info()[0] if cuda else 0
     except Exception:
         free = 0
-    shape = pick_workload(args.workload, free) if (args.workload != "auto" or free) else CONFIGS["C4"]
+    shape = (pick_workload(args.workload, free, args.control) if (args.workload != "auto" or free)
+             else pick_workload("C4", 0, args.control))
+    if args.stars > 0:
+        shape = shape.scaled(args.stars, name=f"{shape.name}[{args.stars} stars]")
     m_full = shape_rows(shape)
     ms = oracle_sample_rows(m_full, args.oracle_rows)
-    a, idx = host.make_rows(shape, 0, ms)
-    steps, warmup = max(1, min(args.steps, 5)), max(1, min(args.warmup, 2))
-    r = time_oracle(shape, m_full, a, idx, steps, warmup)
+    if cuda:
+        from gaia_synth import device as gdev
+        v, i = gdev.make_system(shape, r0=0, r1=ms)
+        a, idx = v.cpu().numpy(), i.cpu().numpy()
+        del v, i
+        torch.cuda.empty_cache()
+    else:
+        if args.oracle_rows <= 0:
+            ms = min(ms, 4_000_000)
+        a, idx = host.make_rows(shape, 0, ms)
+    steps, warmup = max(1, args.steps), max(1, args.warmup)
+    r = time_oracle(shape, m_full, a, idx, steps, warmup, budget_s=150.0)
     line = {"impl": "reference", "metric": "ms_per_lsqr_iteration", "value": r["value"], "unit": "ms",
-            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["value"],
+            "n_gpus": args.gpus, "steps": r["steps_timed"], "warmup": warmup, "ms_per_step": r["value"],
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{shape.name}: {m_full} rows x {shape.n_unknowns} unknowns",
-                       "timed_steps_on_sample": steps},
+                       "steps_requested": args.steps, "steps_timed_on_sample": r["steps_timed"],
+                       "note": "every step is one oracle LSQR iteration on the row sample; the row part is scaled to the "
+                               "workload's rows (cpu_baseline.sample); the loop stops after 150 s"},
             "cpu_baseline": r,
             "e2e": {"value": r["value"], "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -249,10 +303,12 @@ def run_gsr(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     free, total = torch.cuda.mem_get_info()
-    shape = pick_workload(args.workload, free)
+    shape = pick_workload(args.workload, free, args.control)
     if args.stars > 0:
         shape = shape.scaled(args.stars, name=f"{shape.name}[{args.stars} stars]")
     K, W = args.steps, max(args.warmup, 3)
+    if args.mode == "extras":
+        return run_extras(args, shape, dev, rank, world)
 
     vals, idx = gdev.make_system(shape, device=dev)
     m, n = int(vals.shape[0]), shape.n_unknowns
@@ -265,12 +321,20 @@ def run_gsr(args):
     sysm.aprod1(gdev.x_true(shape, device=dev), b)
     torch.cuda.synchronize()
 
-    # ---- warm-up, then EXACTLY K timed iterations
+    # ---- warm-up, then EXACTLY K timed iterations.  Large systems: the per-kernel CUDA events of gsr_profile are on
+    # (two event records per iteration, nothing else changes).  Small, launch-bound systems (matrix <= 256 MB) replay
+    # a CUDA graph, which the per-kernel events would switch off: there the K iterations are timed with profiling
+    # OFF -- the default product path -- and the kernel durations come from a separate, profiled run afterwards.
+    graph_path = m * 224.0 <= 256.0 * 1024 * 1024 and K >= 2
     sysm.lsqr_init(b)
     sysm.lsqr_iterate(W)
+    if graph_path:
+        sysm.lsqr_iterate(K)      # instantiates the K-iteration graph outside the timed region
+        W += K
     torch.cuda.synchronize()
-    sysm.profile(True)
-    sysm.profile_get(1); sysm.profile_get(2)
+    if not graph_path:
+        sysm.profile(True)
+        sysm.profile_get(1); sysm.profile_get(2)
     l0 = sysm.launch_count()
     sampler = ClockSampler(local_rank)
     if rank == 0:
@@ -286,19 +350,29 @@ def run_gsr(args):
     clocks = sampler.stop() if rank == 0 else None
     ms_total = max_over_ranks(e0.elapsed_time(e1), dev)
     launches = sysm.launch_count() - l0
+    kernel_ms_source = "CUDA events around every launch inside the timed region (gsr_profile)"
+    extra = 0
+    if graph_path:
+        extra = min(K, 8)
+        sysm.profile(True)
+        sysm.profile_get(1); sysm.profile_get(2); sysm.profile_get(3)
+        sysm.lsqr_iterate(extra)
+        torch.cuda.synchronize()
+        kernel_ms_source = (f"separate profiled run of {extra} iterations after the timed region (the timed region replays "
+                            "a CUDA graph, which per-kernel events would disable)")
     ap1_ms, ap1_n = sysm.profile_get(1)
     ap2_ms, ap2_n = sysm.profile_get(2)
     fu_ms, fu_n = sysm.profile_get(3)
     sysm.profile(False)
     res = sysm.lsqr_result()
-    assert res.itn == W + K, f"expected {W + K} iterations, ran {res.itn} (istop {res.istop})"
+    assert res.itn == W + K + extra, f"expected {W + K + extra} iterations, ran {res.itn} (istop {res.istop})"
     ms_iter = ms_total / K
 
-    # ---- single aprod launches (median of 10 after 3 warm-ups, CUDA events)
+    # ---- single aprod launches (median of --reps (20) after 3 warm-ups, CUDA events)
     xv = gdev.test_vector(7, 1, n, device=dev)
     yv = torch.zeros(m, dtype=torch.float64, device=dev)
 
-    def median_ms(fn, reps=10, wu=3):
+    def median_ms(fn, reps=max(args.reps, 1), wu=3):
         ts = []
         for i in range(wu + reps):
             a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -316,11 +390,21 @@ def run_gsr(args):
     cands = [("aprod1", ap1_ms, ap1_n), ("aprod2", ap2_ms, ap2_n), ("lsqr_fused", fu_ms, fu_n)]
     dom, dom_ms, dom_n = max(cands, key=lambda c: c[1] * c[2])
     achieved = ab[dom] / (dom_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic(dom, m)
+    # share of the step: durations of the dominant kernel relative to the step, both per iteration
+    per_iter_launches = dom_n / (extra if graph_path else K)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom, m), "peak_source": peak_src,
-                "algorithmic_bytes": ab[dom], "kernel_ms": dom_ms, "launches_timed": dom_n, "share_of_step": dom_ms * dom_n / ms_total,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                "algorithmic_bytes": ab[dom], "kernel_ms": dom_ms, "kernel_ms_source": kernel_ms_source,
+                "launches_timed": dom_n, "share_of_step": dom_ms * per_iter_launches / ms_iter,
                 "frac_of_8TBs": achieved / NOMINAL_HBM_GBS}
-    iter_gbs = ab["iteration"] / (ms_iter * 1e-3) / 1e9
+    # BASELINE.json's metric: the two-pass formula 472 M + 96 n over the time of one iteration.  With the fused pass
+    # (A streamed once) this is an EFFECTIVE figure, not bytes moved; what the fused schedule itself must move is
+    # 240 M + 24 n (matrix pass) + 72 n (the n-length kernels).
+    eff_gbs = ab["iteration"] / (ms_iter * 1e-3) / 1e9
+    fused = fu_n > 0
+    moved = (ab["lsqr_fused"] + 72 * n) if fused else ab["iteration"]
+    moved_gbs = moved / (ms_iter * 1e-3) / 1e9
 
     line = {"metric": "ms_per_lsqr_iteration", "value": ms_iter, "unit": "ms", "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": ms_iter, "higher_is_better": False, "scaling": "weak",
@@ -328,14 +412,24 @@ def run_gsr(args):
             "config": {"workload": f"{shape.name}: {m} rows x {n} unknowns (S={shape.n_stars}, K={shape.n_knots}/axis, "
                                    f"I={shape.n_instr}, G={shape.n_glob})",
                        "matrix_bytes": m * 224, "l2_policy": "inputs (matrix) far larger than L2; no flush",
-                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas"},
-            "iteration_gbs": iter_gbs, "iteration_frac_of_8TBs": iter_gbs / NOMINAL_HBM_GBS,
-            "iteration_frac_of_measured": iter_gbs / peak,
+                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                       "timed_path": "CUDA-graph replay, profiling off" if graph_path else "eager launches, per-kernel events on",
+                       "options": args.option},
+            "iteration_effective_gbs_two_pass_formula": eff_gbs,
+            "iteration_effective_frac_of_8TBs": eff_gbs / NOMINAL_HBM_GBS,
+            "iteration_effective_frac_of_measured": eff_gbs / peak,
+            "iteration_moved_gbs": moved_gbs, "iteration_moved_frac_of_measured": moved_gbs / peak,
+            "iteration_formula_note": "effective = (472 M + 96 n) / time, BASELINE.json's two-pass formula (target >= 0.70 of "
+                                      "8 TB/s); moved = bytes the schedule that ran must move / time (fused: 240 M + 96 n)",
             "aprod1_ms_in_lsqr": ap1_ms, "aprod2_ms_in_lsqr": ap2_ms, "fused_pass_ms_in_lsqr": fu_ms,
             "aprod1_ms_alone": ap1_alone, "aprod2_ms_alone": ap2_alone,
             "aprod1_gbs_alone": ab["aprod1"] / (ap1_alone * 1e-3) / 1e9,
             "aprod2_gbs_alone": ab["aprod2"] / (ap2_alone * 1e-3) / 1e9,
+            "aprod1_frac_of_8TBs_alone": ab["aprod1"] / (ap1_alone * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "aprod2_frac_of_8TBs_alone": ab["aprod2"] / (ap2_alone * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "single_aprod_reps": max(args.reps, 1),
             "gpu_launches": launches, "roofline": roofline, "clocks": clocks,
+            "l2_dies": sysm.instr_acc_info(),
             "lsqr": {"itn": res.itn, "istop": res.istop, "r1norm": res.r1norm, "anorm": res.anorm}}
 
     # ---- CPU baseline: the oracle, as it stands, on a bounded sample (rank 0, N = 1 only)
@@ -353,6 +447,81 @@ def run_gsr(args):
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_extras(args, shape, dev, rank, world):
+    """--mode extras: what sits either side of the LSQR loop, timed through the binding:
+    gsr_colnorms, K iterations of gsr_lsqr and of gsr_lsqr_ex (column-norm preconditioned, with variances), K
+    iterations with covariance pairs registered, and -- for systems up to 2e7 rows -- both solves to convergence.
+    Wall clock around the blocking calls (each synchronises its stream); median of 3 after one warm-up."""
+    import torch
+    import paper_2503_22863_b200 as gsr
+    from gaia_synth import device as gdev
+    K = max(args.steps, 1)
+    vals, idx = gdev.make_system(shape, device=dev)
+    m, n = int(vals.shape[0]), shape.n_unknowns
+    sysm = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx)
+    for opt in args.option:
+        k, v = opt.split("=")
+        sysm.set_option(k, int(v))
+    b = gdev.noise(shape, m, device=dev)
+    sysm.aprod1(gdev.x_true(shape, device=dev), b)
+    x = torch.empty(n, dtype=torch.float64, device=dev)
+    var = torch.empty(n, dtype=torch.float64, device=dev)
+    cn = torch.empty(n, dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+
+    def wall_ms(fn, reps=3, wu=1):
+        ts = []
+        for i in range(wu + reps):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            if i >= wu:
+                ts.append((time.perf_counter() - t0) * 1e3)
+        ts.sort()
+        return ts[len(ts) // 2]
+
+    out = {"mode": "extras", "workload": f"{shape.name}: {m} rows x {n} unknowns", "iterations": K,
+           "options": args.option, "timing": "wall clock around the blocking call, median of 3 after 1 warm-up"}
+    out["colnorms_ms"] = wall_ms(lambda: sysm.colnorms(cn))
+    out["colnorms_stream_gbs"] = m * 224 / (out["colnorms_ms"] * 1e-3) / 1e9
+    out["lsqr_plain_ms_per_iteration"] = wall_ms(lambda: sysm.lsqr(b, x, K)) / K
+    t_pre = wall_ms(lambda: sysm.lsqr_ex(b, x, var=var, precond=True, itnlim=K))
+    out["lsqr_precond_var_ms_per_iteration"] = (t_pre - out["colnorms_ms"]) / K
+    out["lsqr_precond_var_note"] = "column-norm pass (colnorms_ms) subtracted; init included, as for the plain run"
+    pairs = args.cov_pairs or [1_000_000, 10_000_000]
+    g = torch.Generator(device=dev)
+    g.manual_seed(shape.seed)
+    cov_rows = []
+    for npairs in pairs:
+        j1 = torch.randint(0, n, (npairs,), generator=g, device=dev, dtype=torch.int64)
+        j2 = torch.randint(0, n, (npairs,), generator=g, device=dev, dtype=torch.int64)
+        cov = torch.zeros(npairs, dtype=torch.float64, device=dev)
+        sysm.set_cov_pairs(j1, j2, cov)
+        t = wall_ms(lambda: sysm.lsqr_ex(b, x, itnlim=K)) / K
+        sysm.set_cov_pairs(None, None, None)
+        cov_rows.append({"pairs": npairs, "ms_per_iteration": t,
+                         "pairs_alone_ms": t - out["lsqr_plain_ms_per_iteration"],
+                         "list_and_accumulator_gbs": 32.0 * npairs / max((t - out["lsqr_plain_ms_per_iteration"]) * 1e-3, 1e-9) / 1e9})
+        del j1, j2, cov
+    out["cov_pairs"] = cov_rows
+    if m <= 20_000_000:
+        t0 = time.perf_counter()
+        r0 = sysm.lsqr(b, x, 5000, 1e-12, 1e-12, 1e8)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        x0 = x.clone()
+        r1 = sysm.lsqr_ex(b, x, var=var, precond=True, itnlim=5000, atol=1e-12, btol=1e-12, conlim=1e8)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        out["to_convergence"] = {"plain": {"istop": r0.istop, "itn": r0.itn, "wall_ms": (t1 - t0) * 1e3},
+                                 "precond_var": {"istop": r1.istop, "itn": r1.itn, "wall_ms": (t2 - t1) * 1e3},
+                                 "rel_diff_of_x": float(torch.linalg.norm(x - x0) / torch.linalg.norm(x0))}
+    if rank == 0:
+        print(json.dumps(out))
     return 0
 
 

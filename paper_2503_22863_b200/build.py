@@ -33,7 +33,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = SO + ".tmp%d" % os.getpid()
     cmd = [nvcc] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
-    cmd += os.environ.get("GSR_NVCC_EXTRA", "").split()     # experiments only (e.g. -DNAME=value)
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += ["-o", tmp] + sources()
