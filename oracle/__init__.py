@@ -16,12 +16,18 @@ _HDR = os.path.join(_HERE, "gsr_oracle.h")
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (plain C, no FMA contraction)."""
+    """Compile the oracle with gcc (plain C, no FMA contraction).  GSR_ORACLE_SANITIZE=1 builds and loads an
+    AddressSanitizer + UBSan variant instead (run the tests with LD_PRELOAD=$(gcc -print-file-name=libasan.so))."""
+    global _SO
+    flags = ["-O2"]
+    if os.environ.get("GSR_ORACLE_SANITIZE", "0") == "1":
+        _SO = os.path.join(_HERE, "libgsr_oracle_asan.so")
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
     if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(
             os.path.getmtime(_SRC), os.path.getmtime(_HDR)):
         return _SO
     tmp = _SO + ".tmp%d" % os.getpid()
-    subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+    subprocess.check_call(["gcc"] + flags + ["-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
                            "-Wall", "-o", tmp, _SRC, "-lm"])
     os.replace(tmp, _SO)
     return _SO
