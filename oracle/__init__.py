@@ -35,7 +35,7 @@ def build(force: bool = False) -> str:
 
 class Layout(ct.Structure):
     _fields_ = [("n_stars", ct.c_int64), ("n_knots", ct.c_int64), ("n_instr", ct.c_int64),
-                ("n_glob", ct.c_int32)]
+                ("n_glob", ct.c_int32), ("coeffs_per_row", ct.c_int32)]
 
 
 class LsqrResult(ct.Structure):
@@ -146,8 +146,10 @@ def _i(a):
     return a.ctypes.data_as(_ip)
 
 
-def layout(n_stars, n_knots, n_instr, n_glob=1) -> Layout:
-    return Layout(int(n_stars), int(n_knots), int(n_instr), int(n_glob))
+def layout(n_stars, n_knots, n_instr, n_glob=1, coeffs_per_row=24) -> Layout:
+    """coeffs_per_row = 23: the production record without the global slot (needs n_glob = 0)."""
+    assert coeffs_per_row in (23, 24) and (coeffs_per_row == 24 or n_glob == 0)
+    return Layout(int(n_stars), int(n_knots), int(n_instr), int(n_glob), int(coeffs_per_row))
 
 
 def layout_of(shape) -> Layout:
@@ -166,7 +168,7 @@ def col(L: Layout, rec: np.ndarray, k: int) -> int:
 
 def _check(L, a, idx):
     m = a.shape[0]
-    assert a.shape == (m, 24) and idx.shape == (m, 8)
+    assert a.shape == (m, 23 if L.coeffs_per_row == 23 else 24) and idx.shape == (m, 8)
     return m
 
 

@@ -11,6 +11,9 @@
 #endif
 
 #define NSLOT 24  /* N_Astro 5 + N_Att 12 + N_Instr 6 + N_Glob 1 */
+/* Coefficients stored per row = record stride in doubles: 24, or 23 for the production record without the
+ * global slot (N_Glob = 0).  Slots keep their numbers either way. */
+static int nslot_of(const orc_layout *L) { return L->coeffs_per_row == 23 ? 23 : NSLOT; }
 #define NIDX 8    /* {star, att_start, instr[6]}                              */
 
 int orc_max_threads(void) {
@@ -43,11 +46,12 @@ int64_t orc_col(const orc_layout *L, const int32_t *rec, int k) {
 /* Eq. 2: y[r] += sum_k a[r][k] * x[col(r,k)], rows in order, slots in order. */
 void orc_aprod1(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                 const double *x, double *y) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++) {
-    const double *ar = a + r * NSLOT;
+    const double *ar = a + r * ns;
     const int32_t *rec = idx + r * NIDX;
     double s = 0.0;
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, rec, k);
       if (c >= 0) s += ar[k] * x[c];
     }
@@ -59,11 +63,12 @@ void orc_aprod1(const orc_layout *L, int64_t nrows, const double *a, const int32
  * Repeated columns inside one row simply accumulate. */
 void orc_aprod2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                 const double *y, double *x) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++) {
-    const double *ar = a + r * NSLOT;
+    const double *ar = a + r * ns;
     const int32_t *rec = idx + r * NIDX;
     const double yr = y[r];
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, rec, k);
       if (c >= 0) x[c] += ar[k] * yr;
     }
@@ -73,11 +78,12 @@ void orc_aprod2(const orc_layout *L, int64_t nrows, const double *a, const int32
 /* Same sum as orc_aprod2 with Neumaier's compensated accumulation per x entry. */
 void orc_aprod2_comp(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                      const double *y, double *x, double *comp) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++) {
-    const double *ar = a + r * NSLOT;
+    const double *ar = a + r * ns;
     const int32_t *rec = idx + r * NIDX;
     const double yr = y[r];
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, rec, k);
       if (c < 0) continue;
       double t = ar[k] * yr;
@@ -91,11 +97,12 @@ void orc_aprod2_comp(const orc_layout *L, int64_t nrows, const double *a, const 
 
 void orc_aprod1_abs(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                     const double *x, const double *y_in, double *s_out) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++) {
-    const double *ar = a + r * NSLOT;
+    const double *ar = a + r * ns;
     const int32_t *rec = idx + r * NIDX;
     double s = y_in ? fabs(y_in[r]) : 0.0;
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, rec, k);
       if (c >= 0) s += fabs(ar[k] * x[c]);
     }
@@ -111,27 +118,29 @@ void orc_aprod1_abs(const orc_layout *L, int64_t nrows, const double *a, const i
  * column j of A as an operator.  A column can repeat inside a row (instrumental slots): the
  * coefficients of equal columns are summed first, in slot order, and the sum is squared once. */
 void orc_colnorm2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, double *nrm2sq) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++)
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, idx + r * NIDX, k);
       if (c < 0) continue;
       int seen = 0;                         /* an earlier slot of this row already carried column c */
       for (int k0 = 0; k0 < k; k0++)
         if (orc_col(L, idx + r * NIDX, k0) == c) seen = 1;
       if (seen) continue;
-      double arj = a[r * NSLOT + k];        /* A[r][c]: this slot and every later slot on the same column */
-      for (int k1 = k + 1; k1 < NSLOT; k1++)
-        if (orc_col(L, idx + r * NIDX, k1) == c) arj += a[r * NSLOT + k1];
+      double arj = a[r * ns + k];        /* A[r][c]: this slot and every later slot on the same column */
+      for (int k1 = k + 1; k1 < ns; k1++)
+        if (orc_col(L, idx + r * NIDX, k1) == c) arj += a[r * ns + k1];
       nrm2sq[c] += arj * arj;
     }
 }
 /* a_out[r][k] = a[r][k] * s[col(r,k)] : the matrix A diag(s), same index records. */
 void orc_scale_columns(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx, const double *s,
                        double *a_out) {
+  const int ns = nslot_of(L);
   for (int64_t r = 0; r < nrows; r++)
-    for (int k = 0; k < NSLOT; k++) {
+    for (int k = 0; k < ns; k++) {
       int64_t c = orc_col(L, idx + r * NIDX, k);
-      a_out[r * NSLOT + k] = c >= 0 ? a[r * NSLOT + k] * s[c] : a[r * NSLOT + k];
+      a_out[r * ns + k] = c >= 0 ? a[r * ns + k] * s[c] : a[r * ns + k];
     }
 }
 
@@ -152,7 +161,7 @@ void orc_aprod1_omp(const orc_layout *L, int64_t nrows, const double *a, const i
     int t = 0, T = 1;
 #endif
     int64_t r0 = nrows * t / T, r1 = nrows * (t + 1) / T;
-    orc_aprod1(L, r1 - r0, a + r0 * NSLOT, idx + r0 * NIDX, x, y + r0);
+    orc_aprod1(L, r1 - r0, a + r0 * nslot_of(L), idx + r0 * NIDX, x, y + r0);
   }
 }
 
@@ -168,6 +177,7 @@ static int64_t star_aligned(const int32_t *idx, int64_t nrows, int64_t r) {
  * private accumulators that are added to x in thread order (deterministic for fixed T). */
 void orc_aprod2_omp(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                     const double *y, double *x, int threads) {
+  const int ns = nslot_of(L);
   threads = clamp_threads(threads);
   const int64_t oA = 5 * L->n_stars;
   const int64_t nshared = 3 * L->n_knots + L->n_instr + L->n_glob;
@@ -184,10 +194,10 @@ void orc_aprod2_omp(const orc_layout *L, int64_t nrows, const double *a, const i
     int64_t r1 = (t == T - 1) ? nrows : star_aligned(idx, nrows, nrows * (t + 1) / T);
     double *p = priv + (size_t)t * nshared;
     for (int64_t r = r0; r < r1; r++) {
-      const double *ar = a + r * NSLOT;
+      const double *ar = a + r * ns;
       const int32_t *rec = idx + r * NIDX;
       const double yr = y[r];
-      for (int k = 0; k < NSLOT; k++) {
+      for (int k = 0; k < ns; k++) {
         int64_t c = orc_col(L, rec, k);
         if (c < 0) continue;
         if (c < oA) x[c] += ar[k] * yr;

@@ -42,6 +42,8 @@ typedef struct {
   int64_t n_knots;  /* K : attitude block = 3*K columns, axis offset K */
   int64_t n_instr;  /* I                                               */
   int32_t n_glob;   /* 0 or 1 (PAPER.md:141 uses 0, BASELINE configs 1) */
+  int32_t coeffs_per_row; /* record stride in doubles: 0 or 24 = the 24-slot record; 23 = the production record without
+                             the global slot (requires n_glob = 0)                      */
 } orc_layout;
 
 typedef struct {
@@ -54,7 +56,7 @@ int64_t orc_n_unknowns(const orc_layout *L);
 /* column of slot k (0..23) of a row with index record rec[8]; -1 if the slot is unused */
 int64_t orc_col(const orc_layout *L, const int32_t *rec, int k);
 
-/* a: nrows*24 row-major, idx: nrows*8, chunk-local (row 0 of the chunk first). */
+/* a: nrows*24 (or nrows*23, see coeffs_per_row) row-major, idx: nrows*8, chunk-local (row 0 of the chunk first). */
 void orc_aprod1(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,
                 const double *x, double *y);
 void orc_aprod2(const orc_layout *L, int64_t nrows, const double *a, const int32_t *idx,

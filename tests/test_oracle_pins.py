@@ -487,3 +487,76 @@ def test_covariances_of_pairs():
     A5 = a1[:, :5]
     exact = np.linalg.inv(A5.T @ A5)
     assert r5["itn"] == 5 and np.allclose(c5.reshape(5, 5), exact, rtol=1e-8, atol=1e-10 * np.abs(exact).max())
+
+
+# ------------------------------------------------------------------ the 23-coefficient production record
+def _sys23(shape):
+    """A system with N_Glob = 0 in both storages: 24 doubles per row (slot 23 holds junk, which G = 0 must ignore)
+    and the 184-byte production record with the first 23 of them."""
+    assert shape.n_glob == 0
+    a24, idx = host.make_rows(shape)
+    a24[:, 23] = host.test_vector(shape.seed, 9, a24.shape[0])     # junk in the unused global slot
+    a23 = np.ascontiguousarray(a24[:, :23])
+    L24 = oracle.layout_of(shape)
+    L23 = oracle.layout(shape.n_stars, shape.n_knots, shape.n_instr, 0, coeffs_per_row=23)
+    return a24, a23, idx, L24, L23
+
+
+def test_coeff23_record_is_the_dense_matrix_of_its_23_slots():
+    """PAPER.md:141 (N_Glob = 0): the record without the global slot.  Pinned on the dense matrix built by the
+    test-side column map from the 23 stored coefficients alone, entry by entry; and bit-identical to the 24-slot
+    storage of the same system (same slots, same order, only the stride differs)."""
+    shape = tiny_shape(n_stars=6, obs=9, n_knots=10, n_instr=7, n_glob=0, seed=2323)
+    a24, a23, idx, L24, L23 = _sys23(shape)
+    m, n = a23.shape[0], shape.n_unknowns
+    cols = columns_of(shape, idx)
+    assert np.all(cols[:, 23] == -1)
+    D = np.zeros((m, n))
+    for r in range(m):
+        for k in range(23):
+            D[r, cols[r, k]] += a23[r, k]
+    x, y = host.test_vector(2, 1, n), host.test_vector(2, 2, m)
+    y1 = oracle.aprod1(L23, a23, idx, x, np.zeros(m))
+    x1 = oracle.aprod2(L23, a23, idx, y, np.zeros(n))
+    np.testing.assert_allclose(y1, D @ x, rtol=0, atol=1e-13 * np.abs(D).dot(np.abs(x)).max())
+    np.testing.assert_allclose(x1, D.T @ y, rtol=0, atol=1e-13 * np.abs(D.T).dot(np.abs(y)).max())
+    for j in range(n):                                   # a wrong stride shifts every row after the first
+        e = np.zeros(n)
+        e[j] = 1.0
+        np.testing.assert_allclose(oracle.aprod1(L23, a23, idx, e, np.zeros(m)), D[:, j], rtol=0, atol=1e-15)
+    for r in (0, 1, m // 2, m - 1):
+        e = np.zeros(m)
+        e[r] = 1.0
+        np.testing.assert_allclose(oracle.aprod2(L23, a23, idx, e, np.zeros(n)), D[r], rtol=0, atol=1e-15)
+    assert np.array_equal(y1, oracle.aprod1(L24, a24, idx, x, np.zeros(m)))
+    assert np.array_equal(x1, oracle.aprod2(L24, a24, idx, y, np.zeros(n)))
+    assert np.array_equal(oracle.colnorms(L23, a23, idx), oracle.colnorms(L24, a24, idx))
+    np.testing.assert_allclose(oracle.colnorms(L23, a23, idx), np.linalg.norm(D, axis=0), rtol=1e-14, atol=0)
+    with pytest.raises(AssertionError):                  # the binding refuses a 24-wide array for a 23-wide layout
+        oracle.aprod1(L23, a24, idx, x, np.zeros(m))
+
+
+def test_coeff23_omp_compensated_and_lsqr():
+    shape = tiny_shape(n_stars=40, obs=17, n_knots=16, n_instr=9, n_glob=0, seed=2324)
+    a24, a23, idx, L24, L23 = _sys23(shape)
+    m, n = a23.shape[0], shape.n_unknowns
+    x, y = host.test_vector(3, 1, n), host.test_vector(3, 2, m)
+    for th in (2, 3):                                    # chunk offsets of the OpenMP partitions use the stride too
+        assert np.array_equal(oracle.aprod1(L23, a23, idx, x, np.zeros(m), threads=th),
+                              oracle.aprod1(L23, a23, idx, x, np.zeros(m)))
+        np.testing.assert_allclose(oracle.aprod2(L23, a23, idx, y, np.zeros(n), threads=th),
+                                   oracle.aprod2(L23, a23, idx, y, np.zeros(n)), rtol=0, atol=1e-12)
+    comp = np.zeros(n)
+    xc = oracle.aprod2_comp(L23, a23, idx, y, np.zeros(n), comp)
+    np.testing.assert_allclose(xc + comp, oracle.aprod2(L23, a23, idx, y, np.zeros(n)), rtol=0, atol=1e-12)
+    assert np.array_equal(oracle.aprod1_abs(L23, a23, idx, x), oracle.aprod1_abs(L24, a24, idx, x))
+    s = 0.5 + np.abs(host.test_vector(3, 3, n))
+    assert np.array_equal(oracle.scale_columns(L23, a23, idx, s), oracle.scale_columns(L24, a24, idx, s)[:, :23])
+    # LSQR: the same iteration bit for bit in both storages, and the dense least-squares solution
+    b = rhs(shape, a24, idx, host.x_true(shape))
+    x23, r23 = oracle.lsqr(L23, a23, idx, b, itnlim=2000, atol=1e-14, btol=1e-14)
+    x24, r24 = oracle.lsqr(L24, a24, idx, b, itnlim=2000, atol=1e-14, btol=1e-14)
+    assert np.array_equal(x23, x24) and r23 == r24 and r23["istop"] in (1, 2)
+    D = dense_matrix(shape, a24, idx)
+    xr = np.linalg.lstsq(D, b, rcond=None)[0]
+    assert np.linalg.norm(x23 - xr) <= 1e-10 * np.linalg.norm(xr)
