@@ -77,6 +77,11 @@ typedef struct {
                       device-side validation pass (4 ms at 5e8 rows).  Other bits: GSR_EINVAL */
 } gsr_layout;
 #define GSR_LAYOUT_TRUSTED 1
+#define GSR_LAYOUT_COEFF23 2 /* values records hold 23 doubles (184 B): the production record without the global
+                                slot (N_Glob = 0; requires n_glob = 0).  Slots keep their numbers.
+                                First version: served by the one-thread-per-row kernels and the two-pass LSQR
+                                schedule (184-byte rows have no 16-byte alignment and no whole-line row-pair TMA
+                                view); gsr_lsqr_ex with GSR_PRECOND_COLNORM returns GSR_ESTATE for it.             */
 
 typedef struct {
   int32_t istop; /* Paige-Saunders stop code 0..7 (not an error)                      */
@@ -106,6 +111,15 @@ int gsr_create(gsr_system **out, const gsr_layout *layout, const double *values,
                const int32_t *indices, void *stream);
 void gsr_destroy(gsr_system *sys);
 int gsr_dims(const gsr_system *sys, int64_t *n_rows, int64_t *n_unknowns); /* host out-pointers */
+/* gsr_attach_constraints: the constraint equations as a section of their own ("a set of constraints
+ *   equations", "~1 % of the entire system, is replicated among the MPI processes").
+ *   n_rows records in the system's own format (values: n_rows x 24, or x 23 with GSR_LAYOUT_COEFF23; indices:
+ *   n_rows x 8; device, 32-byte aligned, BORROWED until gsr_destroy or the next call), sorted by star among
+ *   themselves, validated like gsr_create's.  The system then has n_rows(create) + n_rows(constraints) rows, the
+ *   constraint rows LAST: every M-vector (y of the products, b of LSQR) carries them after the observation rows.
+ *   Every product and every LSQR pass runs over both sections.  Voids a solve in progress (GSR_ESTATE until the next
+ *   gsr_lsqr_init); n_rows = 0 detaches.  Synchronises `stream` once. */
+int gsr_attach_constraints(gsr_system *sys, int64_t n_rows, const double *values, const int32_t *indices, void *stream);
 
 /* ---- the two products (asynchronous on `stream`) --------------------------------------------
  * gsr_aprod1:  y[r] += sum_k a[r][k] * x[col(r,k)]      Eq. (2).  x: n, y: M.
@@ -149,7 +163,8 @@ int gsr_lsqr_get_state(gsr_system *sys, double *u, double *v, double *w, double 
 /* ---- whole solve from HOST buffers (end-to-end path) ----------------------------------------
  * Allocates device memory, copies values / indices / b host->device, runs gsr_create + gsr_lsqr,
  * copies x device->host, frees everything.  All four arrays are HOST pointers (pinned or
- * pageable); x_host (n) is overwritten.  Blocking. */
+ * pageable; values_host holds 24, or with GSR_LAYOUT_COEFF23 23, doubles per row); x_host (n) is overwritten.
+ * Blocking. */
 int gsr_lsqr_host(const gsr_layout *layout, const double *values_host, const int32_t *indices_host,
                   const double *b_host, double *x_host, int64_t itnlim, double atol, double btol,
                   double conlim, gsr_lsqr_result *res);

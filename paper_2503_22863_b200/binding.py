@@ -52,6 +52,7 @@ class LsqrResult:
 
 GSR_PRECOND_COLNORM = 1
 GSR_LAYOUT_TRUSTED = 1
+GSR_LAYOUT_COEFF23 = 2
 
 _lib = None
 
@@ -59,6 +60,7 @@ _lib = None
 SYMBOLS = {
     "gsr_create": (ct.c_int, [ct.POINTER(_vp), ct.POINTER(_Layout), _vp, _vp, _vp]),
     "gsr_destroy": (None, [_vp]),
+    "gsr_attach_constraints": (ct.c_int, [_vp, ct.c_int64, _vp, _vp, _vp]),
     "gsr_dims": (ct.c_int, [_vp, ct.POINTER(ct.c_int64), ct.POINTER(ct.c_int64)]),
     "gsr_aprod1": (ct.c_int, [_vp, _vp, _vp, _vp]),
     "gsr_aprod2": (ct.c_int, [_vp, _vp, _vp, _vp]),
@@ -138,14 +140,17 @@ class GsrSystem:
 
     values: CUDA float64 [M,24]; indices: CUDA int32 [M,8] -- borrowed, kept alive by this object."""
 
-    def __init__(self, n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False):
+    def __init__(self, n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False, coeffs_per_row=24):
         import torch
         m = int(values.shape[0]) if values is not None else 0
+        if coeffs_per_row not in (23, 24):
+            raise ValueError("coeffs_per_row must be 24 or 23")
+        self.coeffs_per_row = int(coeffs_per_row)
         self.layout = _Layout(m, int(n_stars), int(n_knots), int(n_instr), int(n_glob),
-                              GSR_LAYOUT_TRUSTED if trusted else 0)
+                              (GSR_LAYOUT_TRUSTED if trusted else 0) | (GSR_LAYOUT_COEFF23 if coeffs_per_row == 23 else 0))
         self._values, self._indices = values, indices
         self._h = _vp()
-        vp = _dev_ptr(values, torch.float64, m * 24, "values")
+        vp = _dev_ptr(values, torch.float64, m * self.coeffs_per_row, "values")
         ip = _dev_ptr(indices, torch.int32, m * 8, "indices")
         _check(lib().gsr_create(ct.byref(self._h), ct.byref(self.layout), vp, ip, _stream()), "gsr_create")
         mm, nn = ct.c_int64(), ct.c_int64()
@@ -169,6 +174,18 @@ class GsrSystem:
 
     def __exit__(self, *a):
         self.destroy()
+
+    def attach_constraints(self, values, indices):
+        """The constraint equations as a section of their own (rows after the observation rows); None detaches."""
+        import torch
+        m = int(values.shape[0]) if values is not None else 0
+        _check(lib().gsr_attach_constraints(self._h, m, _dev_ptr(values, torch.float64, m * self.coeffs_per_row, "values"),
+                                            _dev_ptr(indices, torch.int32, m * 8, "indices"), _stream()),
+               "gsr_attach_constraints")
+        self._con_refs = (values, indices)      # borrowed: keep alive
+        mm, nn = ct.c_int64(), ct.c_int64()
+        _check(lib().gsr_dims(self._h, ct.byref(mm), ct.byref(nn)), "gsr_dims")
+        self.n_rows = mm.value
 
     # -- products
     def aprod1(self, x, y):
@@ -272,9 +289,14 @@ class GsrSystem:
 
 
 # ---- free functions with the C names ----------------------------------------------------------
-def gsr_create(n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False) -> GsrSystem:
-    """trusted=True sets GSR_LAYOUT_TRUSTED (the caller vouches for the index records; no validation pass)."""
-    return GsrSystem(n_stars, n_knots, n_instr, n_glob, values, indices, trusted)
+def gsr_create(n_stars, n_knots, n_instr, n_glob, values, indices, trusted=False, coeffs_per_row=24) -> GsrSystem:
+    """trusted=True sets GSR_LAYOUT_TRUSTED (the caller vouches for the index records; no validation pass);
+    coeffs_per_row=23 sets GSR_LAYOUT_COEFF23 (values is [M, 23], n_glob must be 0)."""
+    return GsrSystem(n_stars, n_knots, n_instr, n_glob, values, indices, trusted, coeffs_per_row)
+
+
+def gsr_attach_constraints(sys: GsrSystem, values, indices):
+    sys.attach_constraints(values, indices)
 
 
 def gsr_destroy(sys: GsrSystem):
@@ -314,14 +336,15 @@ def _host_ptr(a, np_dtype, numel, name):
 
 
 def gsr_lsqr_host(n_stars, n_knots, n_instr, n_glob, values, indices, b, x, itnlim, atol=0.0, btol=0.0,
-                  conlim=0.0) -> LsqrResult:
+                  conlim=0.0, coeffs_per_row=24) -> LsqrResult:
     """Whole solve from HOST buffers (H2D copies, create, LSQR, D2H of x inside the call)."""
     import numpy as np
     m = int(values.shape[0])
-    L = _Layout(m, int(n_stars), int(n_knots), int(n_instr), int(n_glob), 0)
+    L = _Layout(m, int(n_stars), int(n_knots), int(n_instr), int(n_glob),
+                GSR_LAYOUT_COEFF23 if coeffs_per_row == 23 else 0)
     n = 5 * L.n_stars + 3 * L.n_knots + L.n_instr + L.n_glob
     r = _Result()
-    _check(lib().gsr_lsqr_host(ct.byref(L), _host_ptr(values, np.float64, m * 24, "values"),
+    _check(lib().gsr_lsqr_host(ct.byref(L), _host_ptr(values, np.float64, m * int(coeffs_per_row), "values"),
                                _host_ptr(indices, np.int32, m * 8, "indices"),
                                _host_ptr(b, np.float64, m, "b"), _host_ptr(x, np.float64, n, "x"),
                                int(itnlim), float(atol), float(btol), float(conlim), ct.byref(r)),

@@ -177,7 +177,8 @@ static cudaError_t launch_tma1(bool gsmem, const SysView& s, const SideData& sd,
   return cudaGetLastError();
 }
 
-// ---- variant 0: one thread per row, direct global loads (simple device-side cross-check) --------
+// ---- variant 0: one thread per row, direct global loads (simple device-side cross-check; the path of the
+// 23-coefficient record, whose 184-byte rows have no 16-byte alignment and no row-pair TMA view) -----------------
 __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const double* __restrict__ x, bool x_il,
                                                           double* __restrict__ y,
                                                           const double* __restrict__ c0p,
@@ -193,16 +194,10 @@ __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const doubl
   double sq = 0.0;
   for (int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; r < s.M;
        r += (int64_t)gridDim.x * blockDim.x) {
-    const double2* ap = reinterpret_cast<const double2*>(s.vals + r * NSLOT);
     const int4* ip = reinterpret_cast<const int4*>(s.idx + r * NIDX);
     const int4 i0 = __ldg(ip), i1 = __ldg(ip + 1);
     double a[NSLOT];
-#pragma unroll
-    for (int q = 0; q < NSLOT / 2; q++) {
-      double2 t = __ldcs(ap + q);
-      a[2 * q] = t.x;
-      a[2 * q + 1] = t.y;
-    }
+    load_record(s, r, a);
     const double* xa = x + 5 * (int64_t)i0.x;
     double acc = 0.0;
 #pragma unroll
@@ -237,7 +232,7 @@ cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t,
                           bool x_il, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
-  if (t.aprod1_variant == 1) {
+  if (t.aprod1_variant == 1 && s.cpr == NSLOT) {   // (the TMA row-pair view needs the 192-byte record)
     const SmemPlan p = plan_smem(s, t, PLAN_APROD1);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const double* att_il = x + s.oA;

@@ -112,27 +112,37 @@ cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, c
   return cudaGetLastError();
 }
 
-// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check) ----
+// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check; the path of the
+// 23-coefficient record).  square = 1: squared column norms (y = 1, coefficients squared; equal columns of a row
+// summed first, reading R22) -----------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const double* __restrict__ y,
                                                           double* __restrict__ x, bool x_il,
                                                           const double* __restrict__ yscale,
-                                                          const int* done) {
+                                                          const int* done, int square) {
   if (done && *done) return;
   const double ys = yscale ? *yscale : 1.0;
   double gsum = 0.0;
   for (int64_t r0 = blockIdx.x * (int64_t)blockDim.x; r0 < s.M; r0 += (int64_t)gridDim.x * blockDim.x) {
     const int64_t r = r0 + threadIdx.x;
     if (r < s.M) {
-      const double2* ap = reinterpret_cast<const double2*>(s.vals + r * NSLOT);
       const int4* ip = reinterpret_cast<const int4*>(s.idx + r * NIDX);
       const int4 i0 = __ldg(ip), i1 = __ldg(ip + 1);
-      const double yr = ys * y[r];
+      const double yr = square ? 1.0 : ys * y[r];
       double a[NSLOT];
+      load_record(s, r, a);
+      if (square) {
+        const int col[6] = {i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+        bool dup[6] = {false, false, false, false, false, false};
 #pragma unroll
-      for (int q = 0; q < NSLOT / 2; q++) {
-        double2 t = __ldcs(ap + q);
-        a[2 * q] = t.x;
-        a[2 * q + 1] = t.y;
+        for (int q = 0; q < 6; q++) {
+          double sum = a[17 + q];
+#pragma unroll
+          for (int p = q + 1; p < 6; p++)
+            if (!dup[q] && col[p] == col[q]) { sum += a[17 + p]; dup[p] = true; }
+          a[17 + q] = dup[q] ? 0.0 : sum;
+        }
+#pragma unroll
+        for (int k = 0; k < NSLOT; k++) a[k] *= a[k];
       }
       double* xa = x + 5 * (int64_t)i0.x;
 #pragma unroll
@@ -165,7 +175,7 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
                           double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
                           int64_t* launches, int square) {
   if (s.M == 0) return cudaSuccess;
-  if (t.aprod2_variant == 1 || square) {
+  if ((t.aprod2_variant == 1 || square) && s.cpr == NSLOT) {   // (the TMA row-pair view needs the 192-byte record)
     const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
@@ -191,7 +201,7 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
   int64_t blocks = (s.M + threads - 1) / threads;
   const int64_t cap = (int64_t)num_sms * 8;
   if (blocks > cap) blocks = cap;
-  k_aprod2_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, y, x, x_il, yscale, done);
+  k_aprod2_rowthread<<<(unsigned)blocks, threads, 0, st>>>(s, y, x, x_il, yscale, done, square);
   ++*launches;
   return cudaGetLastError();
 }

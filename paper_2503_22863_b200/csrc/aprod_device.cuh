@@ -287,6 +287,25 @@ __device__ __forceinline__ double scatter_rest(const RowRegs& r, int lane, bool 
   return gl;
 }
 
+// One thread reads one whole record from global memory (row-thread kernels): 24 doubles as 12 x 128-bit, or the
+// 23 doubles of the production record (184-byte rows: 8-byte alignment only) one by one; slot 23 reads as 0 there.
+__device__ __forceinline__ void load_record(const SysView& s, int64_t r, double (&a)[NSLOT]) {
+  if (s.cpr == NSLOT) {
+    const double2* ap = reinterpret_cast<const double2*>(s.vals + r * NSLOT);
+#pragma unroll
+    for (int q = 0; q < NSLOT / 2; q++) {
+      const double2 t = __ldcs(ap + q);
+      a[2 * q] = t.x;
+      a[2 * q + 1] = t.y;
+    }
+  } else {
+    const double* ap = s.vals + r * (NSLOT - 1);
+#pragma unroll
+    for (int k = 0; k < NSLOT - 1; k++) a[k] = __ldcs(ap + k);
+    a[NSLOT - 1] = 0.0;
+  }
+}
+
 // Shared-memory plan of the TMA kernels.
 struct SmemPlan {
   int warps, stages;

@@ -45,6 +45,10 @@ struct IterGraph;
 struct gsr_system {
   SysView v;
   SideData side;
+  // the constraint equations as a section of their own, rows M .. M + con.M - 1
+  SysView con;
+  SideData con_side;          // its tensor map; every other member aliases `side`
+  bool has_con = false;
   Tuning tune;
   int device = 0;
   int num_sms = 148;
@@ -72,6 +76,9 @@ struct gsr_system {
 };
 
 static inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+static inline int64_t m_total(const gsr_system* s) { return s->v.M + s->con.M; }      // observation + constraint rows
+// one pass over A per LSQR iteration needs the TMA kernels, hence the 192-byte record
+static inline bool fused_path(const gsr_system* s) { return s->tune.fused && s->v.cpr == NSLOT; }
 
 extern "C" const char* gsr_strerror(int code) {
   switch (code) {
@@ -232,7 +239,8 @@ static int check_layout(const gsr_layout* L) {
   if (!L) return GSR_EINVAL;
   if (L->n_rows < 0 || L->n_stars < 1 || L->n_knots < 4 || L->n_instr < 1) return GSR_EINVAL;
   if (L->n_glob != 0 && L->n_glob != 1) return GSR_EINVAL;
-  if (L->flags & ~GSR_LAYOUT_TRUSTED) return GSR_EINVAL;
+  if (L->flags & ~(GSR_LAYOUT_TRUSTED | GSR_LAYOUT_COEFF23)) return GSR_EINVAL;
+  if ((L->flags & GSR_LAYOUT_COEFF23) && L->n_glob != 0) return GSR_EINVAL;   // the 23-slot record has no global slot
   if (L->n_stars > INT32_MAX || L->n_knots > INT32_MAX || L->n_instr > INT32_MAX) return GSR_EINVAL;
   return GSR_OK;
 }
@@ -255,6 +263,9 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
   v.vals = values; v.idx = indices;
   v.M = L->n_rows; v.S = L->n_stars; v.K = L->n_knots; v.I = L->n_instr; v.G = L->n_glob;
   v.oA = 5 * v.S; v.oI = v.oA + 3 * v.K; v.oG = v.oI + v.I; v.n = v.oG + v.G;
+  v.cpr = (L->flags & GSR_LAYOUT_COEFF23) ? NSLOT - 1 : NSLOT;
+  s->con = v;
+  s->con.vals = nullptr; s->con.idx = nullptr; s->con.M = 0;
   // device-side validation of every index record (skipped when the caller vouches for them)
   if (!(L->flags & GSR_LAYOUT_TRUSTED)) {
     int* flag = nullptr;
@@ -271,7 +282,7 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
     if (h != 0) { delete s; return GSR_ELAYOUT; }
   }
   // side structures: the row-tile tensor map, the interleaved attitude buffers, instrumental replicas
-  if (v.M > 0) {
+  if (v.M > 0 && v.cpr == NSLOT) {
     int rc = make_row_tensor_map(&s->side.map, values, v.M);
     if (rc) { delete s; return rc; }
   }
@@ -301,9 +312,44 @@ extern "C" void gsr_destroy(gsr_system* s) {
   delete s;
 }
 
+extern "C" int gsr_attach_constraints(gsr_system* s, int64_t n_rows, const double* values, const int32_t* indices,
+                                      void* stream) {
+  if (!s || n_rows < 0) return GSR_EINVAL;
+  if (n_rows > 0 && (!values || !indices)) return GSR_EINVAL;
+  if (!aligned(values, 32) || !aligned(indices, 32)) return GSR_EINVAL;
+  s->lsqr_ready = false;                 // the row count changes: work vectors are re-made, a running solve is void
+  free_iter_graph(s);
+  cudaFree(s->u); s->u = nullptr;
+  cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->g); cudaFree(s->sc);
+  s->vv = s->w = s->x = s->g = nullptr; s->sc = nullptr;
+  s->has_con = false;
+  s->con.vals = nullptr; s->con.idx = nullptr; s->con.M = 0;
+  if (n_rows == 0) return GSR_OK;
+  SysView c = s->v;
+  c.vals = values; c.idx = indices; c.M = n_rows;
+  int* flag = nullptr;
+  int rc = dev_alloc(reinterpret_cast<void**>(&flag), sizeof(int), "cudaMalloc flag");
+  if (rc) return rc;
+  int h = 0;
+  cudaStream_t st = S(stream);
+  cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), st);
+  if (e == cudaSuccess) e = launch_validate(c, flag, st, &s->launches);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(flag);
+  if (e != cudaSuccess) return cuda_fail(e, "gsr_attach_constraints validation");
+  if (h != 0) return GSR_ELAYOUT;
+  s->con_side = s->side;                 // shares the attitude buffers and the instrumental replicas (never freed twice:
+                                         // gsr_destroy frees `side` only)
+  if (c.cpr == NSLOT && (rc = make_row_tensor_map(&s->con_side.map, values, n_rows))) return rc;
+  s->con = c;
+  s->has_con = true;
+  return GSR_OK;
+}
+
 extern "C" int gsr_dims(const gsr_system* s, int64_t* m, int64_t* n) {
   if (!s) return GSR_EINVAL;
-  if (m) *m = s->v.M;
+  if (m) *m = s->v.M + s->con.M;
   if (n) *n = s->v.n;
   return GSR_OK;
 }
@@ -330,6 +376,8 @@ static int do_aprod1(gsr_system* s, const double* x, bool x_il, double* y, const
   EventPair ep;
   const bool p = prof_begin(s, 1, st, &ep);
   cudaError_t e = launch_aprod1(s->v, s->side, s->tune, s->num_sms, x, x_il, y, c0, sumsq, done, st, &s->launches);
+  if (e == cudaSuccess && s->has_con)   // (a stopped LSQR: the first launch latches done 2 -> 1, this one sees 1)
+    e = launch_aprod1(s->con, s->con_side, s->tune, s->num_sms, x, x_il, y + s->v.M, c0, sumsq, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod1 launch");
   return GSR_OK;
@@ -339,24 +387,26 @@ static int do_aprod2(gsr_system* s, const double* y, double* x, bool x_il, const
   EventPair ep;
   const bool p = prof_begin(s, 2, st, &ep);
   cudaError_t e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, x_il, yscale, done, st, &s->launches);
+  if (e == cudaSuccess && s->has_con)
+    e = launch_aprod2(s->con, s->con_side, s->tune, s->num_sms, y + s->v.M, x, x_il, yscale, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
   if (e != cudaSuccess) return cuda_fail(e, "aprod2 launch");
   return GSR_OK;
 }
 
 extern "C" int gsr_aprod1(gsr_system* s, const double* x, double* y, void* stream) {
-  if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
+  if (!s || !x || (!y && m_total(s) > 0)) return GSR_EINVAL;
   return do_aprod1(s, x, false, y, nullptr, nullptr, nullptr, S(stream));
 }
 extern "C" int gsr_aprod2(gsr_system* s, const double* y, double* x, void* stream) {
-  if (!s || !x || (!y && s->v.M > 0)) return GSR_EINVAL;
+  if (!s || !x || (!y && m_total(s) > 0)) return GSR_EINVAL;
   return do_aprod2(s, y, x, false, nullptr, nullptr, S(stream));
 }
 
 // ---- LSQR ------------------------------------------------------------------------------------
 static int ensure_workspace(gsr_system* s) {
   if (s->sc) return GSR_OK;
-  const size_t m = (size_t)(s->v.M > 0 ? s->v.M : 1), n = (size_t)s->v.n;
+  const size_t m = (size_t)(m_total(s) > 0 ? m_total(s) : 1), n = (size_t)s->v.n;
   cudaError_t e;
   if ((e = cudaMalloc(&s->u, m * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&s->vv, n * sizeof(double))) != cudaSuccess ||
@@ -379,6 +429,8 @@ static int build_dinv(gsr_system* s, cudaStream_t st) {
   if (!s->vs) ALLOC(s->vs, n * sizeof(double));
   CU(cudaMemsetAsync(s->dinv, 0, n * sizeof(double), st));
   CU(launch_aprod2(s->v, s->side, s->tune, s->num_sms, nullptr, s->dinv, true, nullptr, nullptr, st, &s->launches, 1));
+  if (s->has_con)
+    CU(launch_aprod2(s->con, s->con_side, s->tune, s->num_sms, nullptr, s->dinv, true, nullptr, nullptr, st, &s->launches, 1));
   CU(lsqr_launch_colnorm_finish(s->dinv, s->v.n, 1, st, &s->launches));
   return GSR_OK;
 }
@@ -392,7 +444,8 @@ extern "C" int gsr_lsqr_init(gsr_system* s, const double* b, void* stream) {
 }
 
 static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool want_var, void* stream) {
-  if (!s || (!b && s->v.M > 0)) return GSR_EINVAL;
+  if (!s || (!b && m_total(s) > 0)) return GSR_EINVAL;
+  if (precond && !fused_path(s)) return GSR_ESTATE;
   int rc = ensure_workspace(s);
   if (rc) return rc;
   s->opt_precond = precond;
@@ -402,7 +455,7 @@ static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool wan
   s->opt_cov = s->opt_cov_next && s->n_cov > 0;
   if (s->opt_cov) CU(cudaMemsetAsync(s->cov, 0, (size_t)s->n_cov * sizeof(double), S(stream)));
   cudaStream_t st = S(stream);
-  const int64_t M = s->v.M, n = s->v.n;
+  const int64_t M = m_total(s), n = s->v.n;
   CU(cudaMemsetAsync(s->sc, 0, sizeof(DevScalars), st));
   CU(cudaMemsetAsync(s->vv, 0, (size_t)n * sizeof(double), st));
   CU(lsqr_launch_init_u(b, s->u, M, s->sc, st, &s->launches));           // u_hat = b, usq
@@ -426,13 +479,17 @@ static int issue_iterations(gsr_system* s, int64_t n_iters, int64_t itnlim, doub
   const double* dinv = s->opt_precond ? s->dinv : nullptr;
   double* vs = s->opt_precond ? s->vs : nullptr;          // the matrix pass gathers D^-1 v
   double* var = s->opt_var ? s->var : nullptr;
-  for (int64_t it = 0; it < n_iters && s->tune.fused; ++it) {
+  const bool fused = fused_path(s);
+  for (int64_t it = 0; it < n_iters && fused; ++it) {
     // 1+2 in one pass over A: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2 ; g = A^T u_hat
     CU(cudaMemsetAsync(s->g, 0, (size_t)n * sizeof(double), st));
     EventPair ep;
     const bool p = prof_begin(s, 3, st, &ep);
     cudaError_t e = launch_lsqr_fused(s->v, s->side, s->tune, s->num_sms, vs ? vs : s->vv, s->u, s->g, &sc->c0_u,
                                       &sc->usq, &sc->done, st, &s->launches);
+    if (e == cudaSuccess && s->has_con)   // the constraint section: same pass, rows M .. (done: 2 -> 1 latched by the first)
+      e = launch_lsqr_fused(s->con, s->con_side, s->tune, s->num_sms, vs ? vs : s->vv, s->u + s->v.M, s->g, &sc->c0_u,
+                            &sc->usq, &sc->done, st, &s->launches);
     if (p) prof_end(s, st, &ep);
     if (e != cudaSuccess) return cuda_fail(e, "fused LSQR pass launch");
     // beta ; v <- g / beta - beta v ; vsq = ||v||^2
@@ -442,7 +499,7 @@ static int issue_iterations(gsr_system* s, int64_t n_iters, int64_t itnlim, doub
     if (s->opt_cov) CU(lsqr_launch_cov_update(s->v, s->w, sc, s->cov_j1, s->cov_j2, s->n_cov, s->cov, st, &s->launches));
     CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, vs, dinv, var, st, &s->launches));
   }
-  for (int64_t it = 0; it < n_iters && !s->tune.fused; ++it) {
+  for (int64_t it = 0; it < n_iters && !fused; ++it) {
     // 1: u_hat <- A v - (alpha/beta) u_hat ; usq = ||u_hat||^2              (aprod 1)
     int rc = do_aprod1(s, s->vv, true, s->u, &sc->c0_u, &sc->usq, &sc->done, st);
     if (rc) return rc;
@@ -491,7 +548,7 @@ static void free_iter_graph(gsr_system* s) {
 
 // a batch of n_iters iterations is replayed as a CUDA graph (small, launch-bound systems only)
 static bool graph_path(const gsr_system* s, int64_t n_iters) {
-  const bool small = (double)s->v.M * 224.0 <= 256.0 * 1024 * 1024;
+  const bool small = (double)m_total(s) * 224.0 <= 256.0 * 1024 * 1024;
   return s->tune.graph && !s->profile && n_iters >= 2 && small;
 }
 
@@ -499,7 +556,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
                                 double conlim, void* stream) {
   if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
   if (!s->lsqr_ready) return GSR_ESTATE;
-  if (s->opt_precond && !s->tune.fused) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
+  if (s->opt_precond && !fused_path(s)) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
   cudaStream_t st = S(stream);
   if (!graph_path(s, n_iters)) return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
   IterGraph key;
@@ -596,7 +653,7 @@ extern "C" int gsr_lsqr_get_state(gsr_system* s, double* u, double* v, double* w
   if (!s->lsqr_ready) return GSR_ESTATE;
   cudaStream_t st = S(stream);
   int rc;
-  if (u && s->v.M > 0) CU(lsqr_launch_export_u(s->u, u, s->v.M, s->sc, st, &s->launches));
+  if (u && m_total(s) > 0) CU(lsqr_launch_export_u(s->u, u, m_total(s), s->sc, st, &s->launches));
   if (v && (rc = export_nvec(s, s->vv, v, st))) return rc;
   if (w && (rc = export_nvec(s, s->w, w, st))) return rc;
   if (x && (rc = export_nvec(s, s->x, x, st))) return rc;
@@ -646,6 +703,8 @@ extern "C" int gsr_colnorms(gsr_system* s, double* out, void* stream) {
   cudaStream_t st = S(stream);
   CU(cudaMemsetAsync(s->g, 0, (size_t)s->v.n * sizeof(double), st));
   CU(launch_aprod2(s->v, s->side, s->tune, s->num_sms, nullptr, s->g, true, nullptr, nullptr, st, &s->launches, 1));
+  if (s->has_con)
+    CU(launch_aprod2(s->con, s->con_side, s->tune, s->num_sms, nullptr, s->g, true, nullptr, nullptr, st, &s->launches, 1));
   CU(lsqr_launch_colnorm_finish(s->g, s->v.n, 0, st, &s->launches));
   return export_nvec(s, s->g, out, st);
 }
@@ -658,7 +717,7 @@ extern "C" int gsr_lsqr_ex(gsr_system* s, const double* b, double* x, double* va
 static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int32_t flags, int64_t itnlim, double atol,
                     double btol, double conlim, gsr_lsqr_result* res, void* stream, bool with_cov) {
   if (!s || !x || !res || itnlim < 0 || (flags & ~GSR_PRECOND_COLNORM)) return GSR_EINVAL;
-  if ((flags & GSR_PRECOND_COLNORM) && !s->tune.fused) return GSR_ESTATE;
+  if ((flags & GSR_PRECOND_COLNORM) && !fused_path(s)) return GSR_ESTATE;
   s->opt_cov_next = with_cov;   // gsr_lsqr_ex accumulates the registered covariance pairs; gsr_lsqr / gsr_lsqr_init do not
   int rc = lsqr_init_with(s, b, (flags & GSR_PRECOND_COLNORM) != 0, var != nullptr, stream);
   s->opt_cov_next = false;
@@ -700,6 +759,7 @@ extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, con
   if (L->n_rows > 0 && (!values_host || !indices_host || !b_host)) return GSR_EINVAL;
   const size_t M = (size_t)L->n_rows;
   const size_t n = (size_t)(5 * L->n_stars + 3 * L->n_knots + L->n_instr + L->n_glob);
+  const size_t cpr = (L->flags & GSR_LAYOUT_COEFF23) ? NSLOT - 1 : NSLOT;
   double *dv = nullptr, *db = nullptr, *dx = nullptr;
   int32_t* di = nullptr;
   gsr_system* sys = nullptr;
@@ -712,7 +772,7 @@ extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, con
     if (st) cudaStreamDestroy(st);
   };
   if ((e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
-  if ((e = cudaMalloc(&dv, (M ? M : 1) * NSLOT * sizeof(double))) != cudaSuccess ||
+  if ((e = cudaMalloc(&dv, (M ? M : 1) * cpr * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&di, (M ? M : 1) * NIDX * sizeof(int32_t))) != cudaSuccess ||
       (e = cudaMalloc(&db, (M ? M : 1) * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&dx, n * sizeof(double))) != cudaSuccess) {
@@ -722,7 +782,7 @@ extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, con
   }
   if (M) {
     if ((e = cudaMemcpyAsync(di, indices_host, M * NIDX * sizeof(int32_t), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(dv, values_host, M * NSLOT * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dv, values_host, M * cpr * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(db, b_host, M * sizeof(double), cudaMemcpyHostToDevice, st)) != cudaSuccess) {
       cleanup();
       return cuda_fail(e, "cudaMemcpyAsync H2D");

@@ -18,6 +18,7 @@ struct SysView {
   int64_t M, S, K, I;
   int32_t G;
   int64_t oA, oI, oG, n;  // block offsets in x: attitude, instrumental, global; n unknowns
+  int32_t cpr;            // coefficients stored per row = record stride in doubles: 24, or 23 (GSR_LAYOUT_COEFF23, G = 0)
 };
 
 // Device-resident LSQR scalars.  One instance per system.

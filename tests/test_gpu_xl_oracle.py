@@ -30,6 +30,9 @@ from gaia_synth.configs import C4, C5  # noqa: E402
 from gpu_helpers import replay_one_step  # noqa: E402
 
 DEV = "cuda"
+# (module-level so that a dry run of this file's own logic can substitute small cases)
+SLICE_CASE = (C4, 250_000_037, 10_000_011, 1_000_000)      # shape, first row, rows, oracle chunk
+REPLAY_SHAPE = C4
 
 
 def host_ram_available():
@@ -47,8 +50,7 @@ def blocks_of(shape):
 
 def test_c4_slice_aprod_against_streamed_oracle():
     """1e7 contiguous rows of C4 (same K, I, G; the slice starts inside a star and ends on a ragged tile)."""
-    shape = C4
-    r0, nr, chunk = 250_000_037, 10_000_011, 1_000_000
+    shape, r0, nr, chunk = SLICE_CASE
     torch.cuda.empty_cache()
     if torch.cuda.mem_get_info()[0] < (6 << 30):
         pytest.skip("needs 6 GB of HBM")
@@ -82,7 +84,7 @@ def test_c4_slice_aprod_against_streamed_oracle():
             e = np.linalg.norm(got[b] - ref[b])
             assert e <= 1e-11 * nb, f"aprod2 block {name}: {e / nb:.3e}"
         # columns no row of the slice touches stay exactly zero (astrometric columns of the other stars)
-        first_star, last_star = r0 // 100, (r0 + nr - 1) // 100
+        first_star, last_star = r0 // shape.obs_per_star, (r0 + nr - 1) // shape.obs_per_star
         assert not got[:5 * first_star].any() and not got[5 * (last_star + 1):shape.off_att].any()
     del vals, idx
     torch.cuda.empty_cache()
@@ -90,8 +92,8 @@ def test_c4_slice_aprod_against_streamed_oracle():
 
 def test_c4_lsqr_replays_against_oracle():
     """5e8 rows: GPU state at k -> one OpenMP-oracle iteration -> GPU state at k + 1, for k = 0 and k = 10."""
-    shape = C4
-    m, n = 500_000_000, shape.n_unknowns
+    shape = REPLAY_SHAPE
+    m, n = shape.n_stars * shape.obs_per_star, shape.n_unknowns
     need_dev = m * (192 + 32 + 4 * 8) + 12 * n * 8 + (2 << 30)
     need_host = m * (192 + 32 + 3 * 8) + (6 << 30)
     torch.cuda.empty_cache()
