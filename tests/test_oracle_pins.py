@@ -560,3 +560,40 @@ def test_coeff23_omp_compensated_and_lsqr():
     D = dense_matrix(shape, a24, idx)
     xr = np.linalg.lstsq(D, b, rcond=None)[0]
     assert np.linalg.norm(x23 - xr) <= 1e-10 * np.linalg.norm(xr)
+
+
+# ------------------------------------------------------------------ randomised small layouts (hypothesis)
+def test_random_layouts_against_the_dense_matrix():
+    """Any small layout, with or without the global parameter, in either storage, repeated instrumental columns and
+    edge attitude starts included: aprod 1 / aprod 2 / column norms equal the dense matrix built by the test-side
+    column map, and the adjoint identity holds to 1e-13."""
+    hyp = pytest.importorskip("hypothesis")
+    st = pytest.importorskip("hypothesis.strategies")
+
+    @hyp.settings(max_examples=60, deadline=None, derandomize=True)
+    @hyp.given(S=st.integers(1, 5), obs=st.integers(1, 7), K=st.integers(4, 9), I=st.integers(1, 8),
+               G=st.integers(0, 1), cpr=st.sampled_from([24, 23]), seed=st.integers(0, 2 ** 20))
+    def run(S, obs, K, I, G, cpr, seed):
+        if cpr == 23:
+            G = 0
+        rng = np.random.default_rng(seed)
+        m = S * obs
+        shape = SystemShape("rnd", n_stars=S, obs_per_star=obs, n_knots=K, n_instr=I, n_glob=G, seed=seed)
+        a = rng.standard_normal((m, 24))
+        idx = np.empty((m, 8), dtype=np.int32)
+        idx[:, 0] = np.repeat(np.arange(S), obs)
+        idx[:, 1] = rng.integers(0, K - 3, size=m)                # 0 .. K-4 inclusive (the natural bound, R3)
+        idx[:, 2:8] = rng.integers(0, I, size=(m, 6))             # with replacement: repeated columns
+        D = dense_matrix(shape, a, idx)
+        L = oracle.layout(S, K, I, G, coeffs_per_row=cpr)
+        av = np.ascontiguousarray(a[:, :cpr])
+        n = shape.n_unknowns
+        x, y = rng.standard_normal(n), rng.standard_normal(m)
+        ax = oracle.aprod1(L, av, idx, x, np.zeros(m))
+        aty = oracle.aprod2(L, av, idx, y, np.zeros(n))
+        np.testing.assert_allclose(ax, D @ x, rtol=0, atol=1e-13 * (np.abs(D) @ np.abs(x)).max() + 1e-300)
+        np.testing.assert_allclose(aty, D.T @ y, rtol=0, atol=1e-13 * (np.abs(D.T) @ np.abs(y)).max() + 1e-300)
+        assert abs(ax @ y - x @ aty) <= 1e-13 * np.linalg.norm(ax) * np.linalg.norm(y) + 1e-300
+        np.testing.assert_allclose(oracle.colnorms(L, av, idx), np.linalg.norm(D, axis=0), rtol=1e-13, atol=1e-300)
+
+    run()
