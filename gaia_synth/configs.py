@@ -52,12 +52,16 @@ C1 = SystemShape("C1", n_stars=1_000, obs_per_star=20, n_knots=1_000, n_instr=60
 C2 = SystemShape("C2", n_stars=100_000, obs_per_star=100, n_knots=20_000, n_instr=600, seed=SEED_BASE + 2)
 C3 = SystemShape("C3", n_stars=1_000_000, obs_powerlaw=(2.0, 10, 2000), n_knots=200_000,
                  n_instr=6_000, hot_knots=True, seed=SEED_BASE + 3)
+# C3 as BASELINE.json states its size ("mean ~70 ... ~7e7 rows"): the exponent that gives that mean on 10..2000 is 1.83
+# (reading R11; the literal alpha = 2 above gives mean 51.1, ~5.1e7 rows).  Same hot-knot mixture.
+C3B = SystemShape("C3b", n_stars=1_000_000, obs_powerlaw=(1.83, 10, 2000), n_knots=200_000,
+                  n_instr=6_000, hot_knots=True, seed=SEED_BASE + 3)
 C4 = SystemShape("C4", n_stars=5_000_000, obs_per_star=100, n_knots=1_000_000, n_instr=60_000,
                  seed=SEED_BASE + 4)
 C5 = SystemShape("C5", n_stars=2_000_000, obs_per_star=80, n_knots=400_000, n_instr=12_000,
                  n_constraint_rows=10_000, seed=SEED_BASE + 5)
 
-CONFIGS = {c.name: c for c in (C1, C2, C3, C4, C5)}
+CONFIGS = {c.name: c for c in (C1, C2, C3, C3B, C4, C5)}
 
 # stream ids of the counter-based generator (shared by host.py and device.cu)
 STREAM_VALUES = 1
