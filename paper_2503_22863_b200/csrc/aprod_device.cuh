@@ -2,11 +2,11 @@
 // A tile is 32 rows staged in shared memory by TMA (tma.cuh): coefficients as 16 row pairs with a
 // 400-byte pair stride, then the 32 index records.
 //
-// What bounds these kernels on B200 is the number of L2 requests per row (each SM can send one
-// request per cycle to the crossbar, each of the 184 L2 slices looks up one tag per cycle; ncu:
-// l1tex__m_l1tex2xbar_req_cycles_active and lts__t_tag_requests both ~82 % with the previous
-// design), not DRAM bytes.  So every block of a row is handled in the way that needs the fewest
-// requests:
+// What bounds these kernels on B200 at C4 is the number of requests that leave the SM per row (one per clock
+// into the crossbar, an fp64 reduction counting ~1.65), not DRAM bytes and not shared-memory
+// wavefronts (taking 27 of a tile's 267 away changed the fused pass by 0.4 %: shared-memory work runs in the
+// shadow of the requests).  So every block of a row is handled in the way that needs the fewest requests, and
+// whatever can stay in shared memory does:
 //   astro  : lanes of a warp share 1-2 stars -> L1 hits on the gather side; on the scatter side the
 //            per-star sums of a tile are ONE small matrix product (star indicator x coefficients) done
 //            with eight fp64 DMMA.8x8x4, so no shuffles and 2 reduction instructions per tile
