@@ -6,8 +6,11 @@ generation: rows are copied back and fed to it.  Where the oracle can compute an
 outputs are compared one by one with the tolerances of DESIGN.md section 3 (R14, R15).  For the
 shared columns (attitude, instrumental, global), which every row touches, the full-size check is
 the adjoint identity <A x, y> = <x, A^T y> per parameter block (BASELINE.json north_star, 1e-13
-relative) against the aprod 1 that the sampled rows have just verified.  LSQR at full size is
-checked through the residual identity r1norm = ||b - A x|| and a monotone residual.
+relative) against the aprod 1 that the sampled rows have just verified -- a size check, GPU against GPU: the
+same code paths face the ORACLE in full at C2 and at I = 60,000 on a small system (test_gpu_parity.py), and on
+1e7 contiguous rows of the C4 layout block by block in tests/test_gpu_xl_oracle.py.  LSQR at full size is
+checked here through the residual identity r1norm = ||b - A x|| and a monotone residual, and against the oracle
+by one-iteration replays at k = 0 and k = 10 in tests/test_gpu_xl_oracle.py.
 Each case needs the whole system in HBM and is skipped when the device is too small.
 """
 import numpy as np
