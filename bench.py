@@ -228,11 +228,8 @@ def oracle_sample_rows(m_full, requested):
     when the host cannot hold C4), less if host memory is short."""
     if requested > 0:
         return min(requested, m_full)
-    try:
-        import psutil
-        avail = psutil.virtual_memory().available
-    except Exception:
-        avail = 16 << 30
+    from gaia_synth.hostmem import available_host_memory
+    avail = available_host_memory(default=16 << 30)
     cap = int(max(avail * 0.4, 1 << 30) // 260)        # rows + the M-vectors of the oracle's LSQR state
     return max(1, min(m_full, 100_000_000, cap))
 
@@ -544,11 +541,8 @@ def run_e2e(args, shape, sysm, vals, idx, b, m, n, K, dev, rank):
     import numpy as np
     import torch
     import paper_2503_22863_b200 as gsr
-    try:
-        import psutil
-        avail = psutil.virtual_memory().available
-    except Exception:
-        avail = 32 << 30
+    from gaia_synth.hostmem import available_host_memory
+    avail = available_host_memory(default=32 << 30)       # MemAvailable capped by the memory cgroup's headroom
     need = m * 232
     rows = m
     note = "whole workload"

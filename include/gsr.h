@@ -212,8 +212,8 @@ int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_
  *                      die_local         1 (default) L2-resident instrumental accumulators: every CTA reduces into a copy whose
  *                                        4 KB chunks are homed on the L2 of its own die (probed at gsr_create), 0 control
  *                      acc_part, acc_part_fused   when the accumulators live in L2: how many leading instrumental columns are
- *                                        accumulated in left-over shared memory instead (-1 all that fit, 0 none; standalone
- *                                        aprod 2 default -1, fused LSQR pass default 0)
+ *                                        accumulated in left-over shared memory instead (-1 all that fit, 0 none = default of both:
+ *                                        the committed form has not been timed on hardware)
  *                      tab_private       1: the table of die-local chunks is replicated once per shared-memory bank, 0 (default) one copy
  *                      gather_smem       1 (default) stage the instrumental slice of x in shared memory when it fits
  *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x

@@ -6,7 +6,8 @@
 namespace gsr {
 
 // ---- variant 1 (default): TMA-staged row tiles, split by parameter block (aprod_device.cuh) ------
-template <bool ASMEM>
+// PART: see lsqr_fused.cu
+template <bool ASMEM, bool PART>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
              double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
@@ -18,15 +19,17 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
+  if (!PART) acc_part = 0;
   uint32_t* tab_s = reinterpret_cast<uint32_t*>(acc_s + (ASMEM ? 0 : ((acc_part + 1) & ~1)));
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
-  const int64_t n_acc = ASMEM ? s.I : acc_part;   // accumulators privatised in shared memory: all, or the leading columns
-  for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
+  const int64_t n_acc = ASMEM ? s.I : (PART ? acc_part : 0);   // accumulators privatised in shared memory: all, or the leading columns
+  if (ASMEM || PART)
+    for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
   if (!ASMEM && use_tab) load_ins_tab(tab_s, ia, tab_shift);
-  if (n_acc || use_tab) __syncthreads();
+  if (ASMEM || PART || use_tab) __syncthreads();
   ScatterCtx sc{x, gatt_il, x + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr, ia.base, tab_shift, (1 << tab_shift) - 1, acc_part};
   const AttLane al(lane);
   const double ys = yscale ? *yscale : 1.0;
@@ -69,10 +72,10 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     __syncwarp();
     att_scatter(tile, al, ts, gatt_il);
     astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x, square != 0);
-    gacc += scatter_rest<ASMEM>(row, lane, valid, yv, sc);
+    gacc += scatter_rest<ASMEM, PART>(row, lane, valid, yv, sc);
     ring.release(lane);
   }
-  if (n_acc) {
+  if (ASMEM || PART) {
     __syncthreads();
     double* xins = x + s.oI;
     for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) {
@@ -179,14 +182,15 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
     const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
-    auto k = p.acc_smem ? k_aprod2_tma<true> : k_aprod2_tma<false>;
+    const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
+    const bool part = use_copies && p.acc_part > 0;
+    auto k = p.acc_smem ? k_aprod2_tma<true, false> : (part ? k_aprod2_tma<false, true> : k_aprod2_tma<false, false>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
-    const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
     InstrAcc ia = sd.ins;
     if (!t.die_local) ia.two_dies = false;
     k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, y, x, x_il ? x + s.oA : sd.att_acc, ia,
-                                            use_copies ? 1 : 0, p.tab_shift, use_copies ? p.acc_part : 0, yscale, done, square);
+                                            use_copies ? 1 : 0, p.tab_shift, part ? p.acc_part : 0, yscale, done, square);
     ++*launches;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

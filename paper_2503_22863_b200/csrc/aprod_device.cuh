@@ -249,7 +249,7 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
 //  global (slot 23)    : returned as the lane's contribution, reduced once per CTA by the caller.
 //  (Shared memory has no native fp64 add: atomicAdd is an LDS / DADD / ATOMS.CAST.SPIN loop.  Running the
 //  six chains of a row side by side with plain atomicCAS was measured SLOWER: aprod 2 at C2 0.72 vs 0.52 ms.)
-template <bool INSTR_SMEM>
+template <bool INSTR_SMEM, bool PART>
 __device__ __forceinline__ double scatter_rest(const RowRegs& r, int lane, bool valid, double yv, const ScatterCtx& c) {
   double gl = 0.0;
   if (valid) {
@@ -258,20 +258,24 @@ __device__ __forceinline__ double scatter_rest(const RowRegs& r, int lane, bool 
 #pragma unroll
     for (int q = 0; q < 6; q++) inc[q] = r.a[17 + q] * yv;
     if (!INSTR_SMEM && c.ins_tab) {
-      // what bounds the pass at C4 is L2 requests (an fp64 reduction costs ~1.65 of them), and shared-memory work
-      // runs in their shadow: every column that still fits shared memory is accumulated there.  The six L2
-      // reductions stay back to back as predicated instructions (a branch per slot serialised them: +15 %).
       const int lsel = lane & c.tab_mask;
       double* dst[6];
 #pragma unroll
       for (int q = 0; q < 6; q++)
         dst[q] = c.ins_base + c.ins_tab[((col[q] >> INS_CHUNK_SHIFT) << c.tab_shift) | lsel] + (col[q] & (INS_CHUNK - 1));
+      if (PART) {
+        // what bounds the pass at C4 is L2 requests (an fp64 reduction costs ~1.65 of them), and shared-memory work
+        // runs in their shadow: every column that still fits shared memory is accumulated there.  The six L2
+        // reductions stay back to back as predicated instructions (a branch per slot serialised them: +15 %).
+        // PART is a template parameter so that kernels without the partial accumulators carry none of this code.
 #pragma unroll
-      for (int q = 0; q < 6; q++) red_add_if_ge(dst[q], inc[q], col[q], c.acc_part);
-      if (c.acc_part) {
+        for (int q = 0; q < 6; q++) red_add_if_ge(dst[q], inc[q], col[q], c.acc_part);
 #pragma unroll
         for (int q = 0; q < 6; q++)
           if (col[q] < c.acc_part) atomicAdd(c.acc_s + col[q], inc[q]);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 6; q++) red_add(dst[q], inc[q]);
       }
     } else {
       if (INSTR_SMEM) {

@@ -49,10 +49,12 @@ struct Tuning {
   int die_local = 1;       // L2 instrumental accumulators: 1 = each CTA reduces into a copy homed on its own die, 0 = die-0 copies for all (control)
   int gather_smem = 1;     // instrumental slice of x: 1 = staged in shared memory when it fits, 0 = L1/L2 gathers
   // L2 instrumental accumulators: leading columns privatised in whatever shared memory is left (-1 = all that fit,
-  // 0 = none, n = at most n).  Measured at the C4 shape (2e7 rows, profiles/r02_summary.md): standalone aprod 2
-  // 1.363 -> 1.222 ms with 6,000 of the 60,000 columns in shared memory; the fused pass keeps it off until measured
-  // in its predicated form (the first, branchy form cost it +15 %).
-  int acc_part = -1;       // standalone aprod 2
+  // 0 = none, n = at most n); kernels instantiated with PART = true.  Measured at the C4 shape in a first form with a
+  // branch per slot (profiles/r02_summary.md): standalone aprod 2 at 2e7 rows 1.363 -> 1.222 ms with 6,000 of the
+  // 60,000 columns in shared memory, at 5e8 rows 36.8 -> 36.4 ms with 4,000; the fused pass lost 15-40 %.  The
+  // committed form (predicated reductions) has not run on hardware (the GPU pool closed first), so both are OFF by
+  // default: the default kernels are the PART = false instances, instruction for instruction those measured in round 1.
+  int acc_part = 0;        // standalone aprod 2
   int acc_part_fused = 0;  // fused LSQR pass
   int tab_private = 0;     // die-local chunk table: 1 = one copy per shared-memory bank (no LDS bank conflicts; measured -0.4 %:
                            // shared-memory wavefronts are not what bounds the pass), 0 = one copy (leaves 15 KB to acc_part)

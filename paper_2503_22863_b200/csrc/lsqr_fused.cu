@@ -13,7 +13,9 @@
 namespace gsr {
 
 // v and g are LSQR-internal n-vectors: their attitude blocks are in the interleaved layout (aprod_device.cuh).
-template <bool GSMEM, bool ASMEM>
+// PART: with the L2 instrumental accumulators, the leading acc_part columns are accumulated in shared memory instead
+// (a template parameter: the kernel without them carries none of that code).
+template <bool GSMEM, bool ASMEM, bool PART>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
              double* __restrict__ uh, double* __restrict__ g, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
@@ -31,18 +33,20 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   char* ring_mem = smem + (size_t)warp * nstages * STAGE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* acc_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
+  if (!PART) acc_part = 0;
   double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : ((acc_part + 1) & ~1));
   uint32_t* tab_s = reinterpret_cast<uint32_t*>(xi_s + (GSMEM ? ((s.I + 1) & ~1ll) : 0));
 
   TileRing ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
-  const int64_t n_acc = ASMEM ? s.I : acc_part;   // accumulators privatised in shared memory: all, or the leading columns
-  for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
+  const int64_t n_acc = ASMEM ? s.I : (PART ? acc_part : 0);   // accumulators privatised in shared memory: all, or the leading columns
+  if (ASMEM || PART)
+    for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) acc_s[i] = 0.0;
   if (GSMEM)
     for (int64_t i = threadIdx.x; i < s.I; i += blockDim.x) xi_s[i] = __ldg(v + s.oI + i);
   if (!ASMEM && use_tab) load_ins_tab(tab_s, ia, tab_shift);
-  if (n_acc || GSMEM || use_tab) __syncthreads();
+  if (ASMEM || PART || GSMEM || use_tab) __syncthreads();
   const double* att_il = v + s.oA;
   GatherCtx gc{v, att_il, xi_s, v + s.oI, s.G ? __ldg(v + s.oG) : 0.0};
   ScatterCtx sc{g, g + s.oA, g + s.oI, acc_s, (!ASMEM && use_tab) ? tab_s : nullptr, ia.base, tab_shift, (1 << tab_shift) - 1, acc_part};
@@ -81,10 +85,10 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     __syncwarp();
     att_scatter(tile, al, ts, sc.gatt_il);
     astro_scatter(tile, lane, nvalid, valid, row, out, sc.x);
-    gacc += scatter_rest<ASMEM>(row, lane, valid, out, sc);
+    gacc += scatter_rest<ASMEM, PART>(row, lane, valid, out, sc);
     ring.release(lane);
   }
-  if (n_acc) {
+  if (ASMEM || PART) {
     __syncthreads();
     double* gins = g + s.oI;
     for (int64_t i = threadIdx.x; i < n_acc; i += blockDim.x) {
@@ -111,14 +115,15 @@ cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning
   const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
   const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
   void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, InstrAcc, int, int, int, const double*, double*, int*);
-  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true> : k_lsqr_fused<true, false>;
-  else k = p.acc_smem ? k_lsqr_fused<false, true> : k_lsqr_fused<false, false>;
+  const bool part = use_copies && p.acc_part > 0;
+  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true, false> : (part ? k_lsqr_fused<true, false, true> : k_lsqr_fused<true, false, false>);
+  else k = p.acc_smem ? k_lsqr_fused<false, true, false> : (part ? k_lsqr_fused<false, false, true> : k_lsqr_fused<false, false, false>);
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
   if (e != cudaSuccess) return e;
   ++*launches;
   InstrAcc ia = sd.ins;
   if (!t.die_local) ia.two_dies = false;
-  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, ia, use_copies ? 1 : 0, p.tab_shift, use_copies ? p.acc_part : 0, c0, usq, done);
+  k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, v, uh, g, ia, use_copies ? 1 : 0, p.tab_shift, part ? p.acc_part : 0, c0, usq, done);
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (use_copies) return launch_fold_instr(s, sd, g, done, st, launches);

@@ -36,11 +36,9 @@ REPLAY_SHAPE = C4
 
 
 def host_ram_available():
-    try:
-        import psutil
-        return int(psutil.virtual_memory().available)
-    except Exception:
-        return 0
+    """MemAvailable capped by the memory cgroup's headroom (psutil alone does not see a cgroup limit)."""
+    from gaia_synth.hostmem import available_host_memory
+    return available_host_memory(default=0)
 
 
 def blocks_of(shape):
@@ -101,7 +99,7 @@ def test_c4_lsqr_replays_against_oracle():
     if free < need_dev:
         pytest.skip(f"C4 needs {need_dev / 1e9:.0f} GB of HBM, {free / 1e9:.0f} GB free")
     avail = host_ram_available()
-    if avail < need_host:
+    if avail < 1.15 * need_host:
         pytest.skip(f"the oracle needs the rows in host memory: {need_host / 1e9:.0f} GB, {avail / 1e9:.0f} GB available")
     vals, idx = gdev.make_system(shape)
     s = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx)
@@ -140,7 +138,7 @@ def test_c5_to_convergence_against_oracle():
     free = torch.cuda.mem_get_info()[0]
     if free < m_est * 256 + (4 << 30):
         pytest.skip(f"{shape.name} needs {m_est * 256 / 1e9:.0f} GB of HBM")
-    if host_ram_available() < m_est * 250 + (4 << 30):
+    if host_ram_available() < 1.15 * (m_est * 250 + (4 << 30)):
         pytest.skip(f"the oracle needs {m_est * 250 / 1e9:.0f} GB of host memory")
     vals, idx = gdev.make_system(shape)
     s = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx)
