@@ -195,6 +195,45 @@ int gsr_colnorms(gsr_system *sys, double *out, void *stream);
 int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_t flags, int64_t itnlim,
                 double atol, double btol, double conlim, gsr_lsqr_result *res, void *stream);
 
+/* ---- row-sharded LSQR over several GPUs, in phases --------------------------------
+ * PAPER.md:72 "the computation related to a subset of the total number of observations (rows in matrix A) is
+ * assigned to a different MPI process ... the astrometric part ... is distributed over the MPI processes, whereas the
+ * attitude, instrumental, and global parts are replicated"; "two reduce operations per LSQR iteration,
+ * performed at the end of each aprod 1 and aprod 2 call".
+ *
+ * One process per GPU.  Every rank creates its own gsr_system over a contiguous range of rows cut at a star boundary,
+ * with the GLOBAL n_stars / n_knots / n_instr / n_glob (star ids stay global, so the borrowed index records need no
+ * rewriting; a rank's n-vectors have full length and their astrometric entries outside its own stars stay exactly 0).
+ * The constraint section, if any, is attached on ONE rank.  The library does all the arithmetic of a phase on the
+ * rank's rows; what the ranks must add up between two phases is the first *xcount doubles of the exchange buffer
+ * `xbuf` (device, gsr_shard_exchange_len() doubles = 3K + I + G + 2, caller-owned, borrowed until the solve ends):
+ * the caller sums them over the ranks IN PLACE (one NCCL allreduce(sum) on `stream`) before the next phase call.
+ * Because aprod 1 and aprod 2 of an iteration share one pass over A here, an iteration needs ONE vector reduce (the
+ * replicated tail of A^T u, 24.5 MB at C4, with sum u^2 and sum w^2 riding along) and one scalar reduce (sum v^2)
+ * instead of the paper's two vector reduces.  Every rank then evaluates the same scalars and the same stopping rule.
+ *
+ *   gsr_shard_begin : start a solve of min ||A x - b|| with b = this rank's rows of the right-hand side.
+ *                     counts_shared = 1 on exactly ONE rank (the replicated tail of v and w enters the norms once),
+ *                     0 on the others.  Runs phase 0 (u = b, partial sum b^2); *xcount = 1.
+ *   gsr_shard_phase : run the next phase; *xcount = doubles of xbuf to sum over the ranks before the next call
+ *                     (0 = nothing to exchange); *status = GSR_SHARD_MORE, GSR_SHARD_INIT_DONE (x = 0, v, w set up) or
+ *                     GSR_SHARD_ITER_DONE (one more LSQR iteration complete).  Phases: init b, c, d, then a, b, c of
+ *                     every iteration.  Asynchronous; iterations after a stop are no-ops, as in gsr_lsqr_iterate.
+ *   gsr_shard_poll  : *stopped = 1 once a stopping rule has fired (same value on every rank); *res (host, may be
+ *                     NULL) as gsr_lsqr.  Synchronises `stream`.  The solution is read with gsr_lsqr_result_get: the
+ *                     astrometric block holds this rank's stars (0 elsewhere: the sum over ranks is the whole block),
+ *                     the other blocks are identical on every rank.
+ * Plain LSQR on the one-pass schedule only (GSR_ESTATE with option fused=0 or GSR_LAYOUT_COEFF23); gsr_lsqr_iterate
+ * returns GSR_ESTATE while a sharded solve is in progress; gsr_lsqr_init / gsr_lsqr end it.                          */
+#define GSR_SHARD_MORE 0
+#define GSR_SHARD_INIT_DONE 1
+#define GSR_SHARD_ITER_DONE 2
+int gsr_shard_exchange_len(const gsr_system *sys, int64_t *n_doubles);
+int gsr_shard_begin(gsr_system *sys, const double *b, double *xbuf, int32_t counts_shared, int64_t itnlim, double atol,
+                    double btol, double conlim, int64_t *xcount, void *stream);
+int gsr_shard_phase(gsr_system *sys, int64_t *xcount, int32_t *status, void *stream);
+int gsr_shard_poll(gsr_system *sys, int32_t *stopped, gsr_lsqr_result *res, void *stream);
+
 /* ---- diagnostics ----------------------------------------------------------------------------
  * gsr_launch_count : kernels launched by this system object so far (host out-pointer).
  * gsr_profile      : enable (1) / disable (0) CUDA-event timing of the matrix-pass kernels issued by

@@ -51,6 +51,7 @@ class LsqrResult:
 
 
 GSR_PRECOND_COLNORM = 1
+GSR_SHARD_MORE, GSR_SHARD_INIT_DONE, GSR_SHARD_ITER_DONE = 0, 1, 2
 GSR_LAYOUT_TRUSTED = 1
 GSR_LAYOUT_COEFF23 = 2
 
@@ -76,6 +77,11 @@ SYMBOLS = {
     "gsr_lsqr_get_state": (ct.c_int, [_vp, _vp, _vp, _vp, _vp, ct.POINTER(_Scalars), _vp]),
     "gsr_lsqr_host": (ct.c_int, [ct.POINTER(_Layout), _vp, _vp, _vp, _vp, ct.c_int64, ct.c_double,
                                  ct.c_double, ct.c_double, ct.POINTER(_Result)]),
+    "gsr_shard_exchange_len": (ct.c_int, [_vp, ct.POINTER(ct.c_int64)]),
+    "gsr_shard_begin": (ct.c_int, [_vp, _vp, _vp, ct.c_int32, ct.c_int64, ct.c_double, ct.c_double, ct.c_double,
+                                   ct.POINTER(ct.c_int64), _vp]),
+    "gsr_shard_phase": (ct.c_int, [_vp, ct.POINTER(ct.c_int64), ct.POINTER(ct.c_int32), _vp]),
+    "gsr_shard_poll": (ct.c_int, [_vp, ct.POINTER(ct.c_int32), ct.POINTER(_Result), _vp]),
     "gsr_launch_count": (ct.c_int, [_vp, ct.POINTER(ct.c_int64)]),
     "gsr_profile": (ct.c_int, [_vp, ct.c_int]),
     "gsr_profile_get": (ct.c_int, [_vp, ct.c_int, ct.POINTER(ct.c_double), ct.POINTER(ct.c_int64)]),
@@ -264,6 +270,37 @@ class GsrSystem:
                                         _dev_ptr(x, torch.float64, self.n_unknowns, "x"),
                                         ct.byref(sc), _stream()), "gsr_lsqr_get_state")
         return {k: getattr(sc, k) for k, _ in _Scalars._fields_}
+
+    # -- row-sharded solve in phases (gsr_shard_*; driven by sharded.ShardedLsqr)
+    def shard_exchange_len(self) -> int:
+        n = ct.c_int64()
+        _check(lib().gsr_shard_exchange_len(self._h, ct.byref(n)), "gsr_shard_exchange_len")
+        return n.value
+
+    def exchange_buffer(self):
+        """A device buffer of the size gsr_shard_begin wants (device memory: PyTorch's part of the job)."""
+        import torch
+        return torch.zeros(self.shard_exchange_len(), dtype=torch.float64, device="cuda")
+
+    def shard_begin(self, b, xbuf, counts_shared, itnlim, atol=0.0, btol=0.0, conlim=0.0) -> int:
+        import torch
+        cnt = ct.c_int64()
+        _check(lib().gsr_shard_begin(self._h, _dev_ptr(b, torch.float64, self.n_rows, "b"),
+                                     _dev_ptr(xbuf, torch.float64, self.shard_exchange_len(), "xbuf"),
+                                     int(bool(counts_shared)), int(itnlim), float(atol), float(btol), float(conlim),
+                                     ct.byref(cnt), _stream()), "gsr_shard_begin")
+        self._shard_refs = (b, xbuf)        # borrowed: keep alive
+        return cnt.value
+
+    def shard_phase(self):
+        cnt, status = ct.c_int64(), ct.c_int32()
+        _check(lib().gsr_shard_phase(self._h, ct.byref(cnt), ct.byref(status), _stream()), "gsr_shard_phase")
+        return cnt.value, status.value
+
+    def shard_poll(self):
+        stopped, r = ct.c_int32(), _Result()
+        _check(lib().gsr_shard_poll(self._h, ct.byref(stopped), ct.byref(r), _stream()), "gsr_shard_poll")
+        return bool(stopped.value), _result(r)
 
     # -- diagnostics
     def launch_count(self) -> int:

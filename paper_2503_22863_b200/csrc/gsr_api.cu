@@ -67,6 +67,12 @@ struct gsr_system {
   double* cov = nullptr;
   int64_t n_cov = 0;
   bool opt_cov = false, opt_cov_next = false;              // (opt_cov_next: set by gsr_lsqr_ex for its own init)
+  // row-sharded solve in phases (gsr_shard_*); -1 = none in progress
+  int shard_next = -1;                                     // the phase the next gsr_shard_phase call runs
+  bool shard_counts_shared = false;                        // this rank counts the replicated tail in the sums of squares
+  double* shard_xbuf = nullptr;                            // borrowed exchange buffer (n - 5S + 2 doubles)
+  int64_t shard_itnlim = 0;
+  double shard_atol = 0, shard_btol = 0, shard_conlim = 0;
   // profiling
   bool profile = false;
   std::vector<EventPair> pending;
@@ -318,6 +324,7 @@ extern "C" int gsr_attach_constraints(gsr_system* s, int64_t n_rows, const doubl
   if (n_rows > 0 && (!values || !indices)) return GSR_EINVAL;
   if (!aligned(values, 32) || !aligned(indices, 32)) return GSR_EINVAL;
   s->lsqr_ready = false;                 // the row count changes: work vectors are re-made, a running solve is void
+  s->shard_next = -1;
   free_iter_graph(s);
   cudaFree(s->u); s->u = nullptr;
   cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->g); cudaFree(s->sc);
@@ -448,6 +455,7 @@ static int lsqr_init_with(gsr_system* s, const double* b, bool precond, bool wan
   if (precond && !fused_path(s)) return GSR_ESTATE;
   int rc = ensure_workspace(s);
   if (rc) return rc;
+  s->shard_next = -1;                      // (a sharded solve in progress is void)
   s->opt_precond = precond;
   s->opt_var = want_var;
   if (precond && (rc = build_dinv(s, S(stream)))) return rc;
@@ -556,6 +564,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
                                 double conlim, void* stream) {
   if (!s || n_iters < 0 || itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
   if (!s->lsqr_ready) return GSR_ESTATE;
+  if (s->shard_next >= 0) return GSR_ESTATE;                 // a sharded solve advances through gsr_shard_phase only
   if (s->opt_precond && !fused_path(s)) return GSR_ESTATE;   // the preconditioned operator exists on the fused path only
   cudaStream_t st = S(stream);
   if (!graph_path(s, n_iters)) return issue_iterations(s, n_iters, itnlim, atol, btol, conlim, st);
@@ -750,6 +759,121 @@ static int lsqr_run(gsr_system* s, const double* b, double* x, double* var, int3
     if ((rc = export_nvec(s, src, var, st))) return rc;
   }
   return gsr_lsqr_result_get(s, x, res, stream);
+}
+
+// ---- row-sharded LSQR in phases -----------------------------------
+// The same kernels as gsr_lsqr_init / gsr_lsqr_iterate, cut where a sum over the ranks is needed.  What travels is
+// the replicated tail of g (or v) and the partial sums of squares, through the caller's exchange buffer; the
+// astrometric part of every n-vector is non-zero on its owner only and never travels.
+enum { SH_INIT_B = 1, SH_INIT_C = 2, SH_INIT_D = 3, SH_ITER_A = 4, SH_ITER_B = 5, SH_ITER_C = 6 };
+
+extern "C" int gsr_shard_exchange_len(const gsr_system* s, int64_t* n_doubles) {
+  if (!s || !n_doubles) return GSR_EINVAL;
+  *n_doubles = (s->v.n - s->v.oA) + 2;
+  return GSR_OK;
+}
+
+extern "C" int gsr_shard_begin(gsr_system* s, const double* b, double* xbuf, int32_t counts_shared, int64_t itnlim,
+                               double atol, double btol, double conlim, int64_t* xcount, void* stream) {
+  if (!s || !xbuf || !xcount || (!b && m_total(s) > 0)) return GSR_EINVAL;
+  if (itnlim < 0 || !(atol >= 0) || !(btol >= 0) || !(conlim >= 0)) return GSR_EINVAL;
+  if (!fused_path(s)) return GSR_ESTATE;              // the phases are those of the one-pass schedule
+  int rc = ensure_workspace(s);
+  if (rc) return rc;
+  s->lsqr_ready = false;
+  s->opt_precond = s->opt_var = s->opt_cov = false;
+  s->shard_xbuf = xbuf;
+  s->shard_counts_shared = counts_shared != 0;
+  s->shard_itnlim = itnlim; s->shard_atol = atol; s->shard_btol = btol; s->shard_conlim = conlim;
+  cudaStream_t st = S(stream);
+  const int64_t M = m_total(s), n = s->v.n;
+  CU(cudaMemsetAsync(s->sc, 0, sizeof(DevScalars), st));
+  CU(cudaMemsetAsync(s->vv, 0, (size_t)n * sizeof(double), st));
+  CU(lsqr_launch_init_u(b, s->u, M, s->sc, st, &s->launches));                               // u_hat = b ; partial sum b^2
+  CU(lsqr_launch_shard_xfer(nullptr, 0, s->sc, xbuf, SHARD_X_USQ, 0, st, &s->launches));     // -> xbuf[0]
+  *xcount = 1;
+  s->shard_next = SH_INIT_B;
+  return GSR_OK;
+}
+
+extern "C" int gsr_shard_phase(gsr_system* s, int64_t* xcount, int32_t* status, void* stream) {
+  if (!s || !xcount || !status) return GSR_EINVAL;
+  if (s->shard_next < 0) return GSR_ESTATE;
+  cudaStream_t st = S(stream);
+  DevScalars* sc = s->sc;
+  double* xb = s->shard_xbuf;
+  const int64_t n = s->v.n, oA = s->v.oA, ns = n - oA;
+  const int64_t n_sq = s->shard_counts_shared ? n : oA;     // the replicated tail is counted by one rank only
+  int rc;
+  *xcount = 0;
+  *status = GSR_SHARD_MORE;
+  switch (s->shard_next) {
+    case SH_INIT_B:   // beta = ||b|| ; v = A^T u (this rank's rows)                        exchange: the tail of v
+      CU(lsqr_launch_shard_xfer(nullptr, 0, sc, xb, SHARD_X_USQ, 1, st, &s->launches));
+      CU(lsqr_launch_init_s1(sc, st, &s->launches));
+      if ((rc = do_aprod2(s, s->u, s->vv, true, &sc->s_y, nullptr, st))) return rc;
+      CU(lsqr_launch_shard_xfer(s->vv + oA, ns, sc, xb, SHARD_X_NONE, 0, st, &s->launches));
+      *xcount = ns;
+      s->shard_next = SH_INIT_C;
+      break;
+    case SH_INIT_C:   // partial ||v||^2                                                    exchange: one scalar
+      CU(lsqr_launch_shard_xfer(s->vv + oA, ns, sc, xb, SHARD_X_NONE, 1, st, &s->launches));
+      CU(lsqr_launch_sumsq_v(s->vv, n, sc, nullptr, st, &s->launches, n_sq));
+      CU(lsqr_launch_shard_xfer(nullptr, 0, sc, xb, SHARD_X_VSQ, 0, st, &s->launches));
+      *xcount = 1;
+      s->shard_next = SH_INIT_D;
+      break;
+    case SH_INIT_D:   // alpha ; v /= alpha ; w = v ; x = 0 ; partial ||w||^2 (travels with the first iteration)
+      CU(lsqr_launch_shard_xfer(nullptr, 0, sc, xb, SHARD_X_VSQ, 1, st, &s->launches));
+      CU(lsqr_launch_init_s2(sc, st, &s->launches));
+      CU(lsqr_launch_init_vw(s->vv, s->w, s->x, n, sc, nullptr, nullptr, nullptr, st, &s->launches, n_sq));
+      s->lsqr_ready = true;
+      *status = GSR_SHARD_INIT_DONE;
+      s->shard_next = SH_ITER_A;
+      break;
+    case SH_ITER_A: {  // the fused pass over this rank's rows                 exchange: tail of g, sum u^2, sum w^2
+      CU(cudaMemsetAsync(s->g, 0, (size_t)n * sizeof(double), st));
+      cudaError_t e = launch_lsqr_fused(s->v, s->side, s->tune, s->num_sms, s->vv, s->u, s->g, &sc->c0_u, &sc->usq,
+                                        &sc->done, st, &s->launches);
+      if (e == cudaSuccess && s->has_con)
+        e = launch_lsqr_fused(s->con, s->con_side, s->tune, s->num_sms, s->vv, s->u + s->v.M, s->g, &sc->c0_u, &sc->usq,
+                              &sc->done, st, &s->launches);
+      if (e != cudaSuccess) return cuda_fail(e, "fused LSQR pass launch");
+      CU(lsqr_launch_shard_xfer(s->g + oA, ns, sc, xb, SHARD_X_USQ_WSQ, 0, st, &s->launches));
+      *xcount = ns + 2;
+      s->shard_next = SH_ITER_B;
+      break;
+    }
+    case SH_ITER_B:   // beta ; v <- g / beta - beta v ; partial ||v||^2                    exchange: one scalar
+      CU(lsqr_launch_shard_xfer(s->g + oA, ns, sc, xb, SHARD_X_USQ_WSQ, 1, st, &s->launches));
+      CU(lsqr_launch_vcombine(s->vv, s->g, n, sc, nullptr, st, &s->launches, n_sq));
+      CU(lsqr_launch_shard_xfer(nullptr, 0, sc, xb, SHARD_X_VSQ, 0, st, &s->launches));
+      *xcount = 1;
+      s->shard_next = SH_ITER_C;
+      break;
+    case SH_ITER_C:   // scalars and stopping rule (identical on every rank) ; x, w, v update ; partial ||w||^2
+      CU(lsqr_launch_shard_xfer(nullptr, 0, sc, xb, SHARD_X_VSQ, 1, st, &s->launches));
+      CU(lsqr_launch_step_scalars(sc, s->shard_itnlim, s->shard_atol, s->shard_btol, s->shard_conlim, st, &s->launches));
+      CU(lsqr_launch_update(s->vv, s->w, s->x, n, sc, nullptr, nullptr, nullptr, st, &s->launches, n_sq));
+      *status = GSR_SHARD_ITER_DONE;
+      s->shard_next = SH_ITER_A;
+      break;
+    default:
+      return GSR_ESTATE;
+  }
+  return GSR_OK;
+}
+
+extern "C" int gsr_shard_poll(gsr_system* s, int32_t* stopped, gsr_lsqr_result* res, void* stream) {
+  if (!s || !stopped) return GSR_EINVAL;
+  if (s->shard_next < 0 || !s->lsqr_ready) return GSR_ESTATE;
+  DevScalars h;
+  int rc = fetch_scalars(s, &h, S(stream));
+  if (rc) return rc;
+  if (!h.done && s->shard_itnlim == 0) { h.done = 1; h.istop = 7; }   // as gsr_lsqr with itnlim = 0: no iteration is allowed
+  *stopped = h.done ? 1 : 0;
+  if (res) fill_result(h, res);
+  return GSR_OK;
 }
 
 extern "C" int gsr_lsqr_host(const gsr_layout* L, const double* values_host, const int32_t* indices_host,

@@ -115,22 +115,23 @@ cudaError_t launch_att_from_il(const SysView& s, int num_sms, const double* il, 
                                int64_t* launches);
 cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, const int* done, cudaStream_t st,
                               int64_t* launches);
+// (n_sq: how many leading elements enter the kernel's sum of squares; -1 = all n.  Only a row-sharded solve passes less.)
 cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, const double* dinv,
-                                 cudaStream_t st, int64_t* launches);
+                                 cudaStream_t st, int64_t* launches, int64_t n_sq = -1);
 
 // LSQR vector / scalar kernels (lsqr_kernels.cu)
 cudaError_t lsqr_launch_init_u(const double* b, double* u, int64_t M, DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_sumsq_v(double* v, int64_t n, DevScalars* sc, const double* dinv, cudaStream_t st,
-                                int64_t* launches);
+                                int64_t* launches, int64_t n_sq = -1);
 cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
-                                const double* dinv, double* var, cudaStream_t st, int64_t* launches);
+                                const double* dinv, double* var, cudaStream_t st, int64_t* launches, int64_t n_sq = -1);
 cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
                                      cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
-                               const double* dinv, double* var, cudaStream_t st, int64_t* launches);
+                               const double* dinv, double* var, cudaStream_t st, int64_t* launches, int64_t n_sq = -1);
 cudaError_t lsqr_launch_cov_update(const SysView& s, const double* w, const DevScalars* sc, const int64_t* j1,
                                    const int64_t* j2, int64_t n_pairs, double* cov, cudaStream_t st, int64_t* launches);
 cudaError_t lsqr_launch_cov_unscale(const SysView& s, const double* dinv, const int64_t* j1, const int64_t* j2,
@@ -141,6 +142,10 @@ cudaError_t lsqr_launch_colnorm_finish(double* d, int64_t n, int mode, cudaStrea
 cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s, int64_t n, int power, cudaStream_t st,
                                  int64_t* launches);
 cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches);
+// row-sharded solve: which partial sums travel with the exchange buffer (lsqr_kernels.cu, k_shard_xfer)
+enum { SHARD_X_NONE = 0, SHARD_X_USQ = 1, SHARD_X_VSQ = 2, SHARD_X_USQ_WSQ = 3 };
+cudaError_t lsqr_launch_shard_xfer(double* vec, int64_t ns, DevScalars* sc, double* xbuf, int what, int unpack,
+                                   cudaStream_t st, int64_t* launches);
 
 // ---- device helpers -----------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double v) {

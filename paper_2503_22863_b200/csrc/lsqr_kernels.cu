@@ -45,15 +45,17 @@ __global__ void k_init_s1(DevScalars* sc) {
 }
 
 // vsq = ||v||^2; with a preconditioner, v <- D^-1 v first (v = A^T u becomes (A D^-1)^T u)
+// n_sq (here and in the three n-length kernels below): only elements i < n_sq enter the sum of squares.  n_sq = n
+// except in a row-sharded solve (gsr_shard_*), where the replicated tail of the vector is counted by one rank only.
 __global__ void __launch_bounds__(256) k_sumsq_v(double* __restrict__ v, int64_t n, DevScalars* sc,
-                                                 const double* __restrict__ dinv) {
+                                                 const double* __restrict__ dinv, int64_t n_sq) {
   if (sc->done) return;
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
        i += (int64_t)gridDim.x * blockDim.x) {
     double t = v[i];
     if (dinv) { t *= dinv[i]; v[i] = t; }
-    sq = fma(t, t, sq);
+    if (i < n_sq) sq = fma(t, t, sq);
   }
   sq = block_sum(sq);
   if (threadIdx.x == 0) atomicAdd(&sc->vsq, sq);
@@ -81,7 +83,7 @@ __global__ void k_init_s2(DevScalars* sc) {
 __global__ void __launch_bounds__(256) k_init_vw(double* __restrict__ v, double* __restrict__ w,
                                                  double* __restrict__ x, int64_t n, DevScalars* sc,
                                                  double* __restrict__ vs, const double* __restrict__ dinv,
-                                                 double* __restrict__ var) {
+                                                 double* __restrict__ var, int64_t n_sq) {
   const double ia = sc->inv_alpha;
   double sq = 0.0;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
@@ -92,7 +94,7 @@ __global__ void __launch_bounds__(256) k_init_vw(double* __restrict__ v, double*
     x[i] = 0.0;
     if (vs) vs[i] = t * dinv[i];
     if (var) var[i] = 0.0;
-    sq = fma(t, t, sq);
+    if (i < n_sq) sq = fma(t, t, sq);
   }
   sq = block_sum(sq);
   if (threadIdx.x == 0) atomicAdd(&sc->wsq, sq);
@@ -119,7 +121,7 @@ __global__ void __launch_bounds__(256) k_vscale(double* __restrict__ v, int64_t 
 // g = A^T u_hat was accumulated by the fused pass.  Thread 0 publishes beta, 1/beta and anorm.
 // With a preconditioner g holds A^T u_hat and the operator's transpose is D^-1 A^T: g is scaled on the fly.
 __global__ void __launch_bounds__(256) k_vcombine(double* __restrict__ v, const double* __restrict__ g, int64_t n,
-                                                  DevScalars* sc, const double* __restrict__ dinv) {
+                                                  DevScalars* sc, const double* __restrict__ dinv, int64_t n_sq) {
   if (sc->done) return;
   const double beta = sqrt(sc->usq);
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -135,7 +137,7 @@ __global__ void __launch_bounds__(256) k_vcombine(double* __restrict__ v, const 
     const double gi = dinv ? g[i] * dinv[i] : g[i];
     const double t = fma(nb, v[i], gi * ib);
     v[i] = t;
-    sq = fma(t, t, sq);
+    if (i < n_sq) sq = fma(t, t, sq);
   }
   sq = block_sum(sq);
   if (threadIdx.x == 0) atomicAdd(&sc->vsq, sq);
@@ -206,7 +208,7 @@ __global__ void k_step_scalars(DevScalars* sc, int64_t itnlim, double atol, doub
 __global__ void __launch_bounds__(256) k_update(double* __restrict__ v, double* __restrict__ w,
                                                 double* __restrict__ x, int64_t n, DevScalars* sc,
                                                 double* __restrict__ vs, const double* __restrict__ dinv,
-                                                double* __restrict__ var) {
+                                                double* __restrict__ var, int64_t n_sq) {
   if (sc->done == 1) return;
   const double ia = sc->inv_alpha, t1 = sc->t1, t2 = sc->t2, ir = sc->inv_rho;
   double sq = 0.0;
@@ -219,7 +221,7 @@ __global__ void __launch_bounds__(256) k_update(double* __restrict__ v, double* 
     x[i] = fma(t1, wi, x[i]);
     const double wn = fma(t2, wi, vi);
     w[i] = wn;
-    sq = fma(wn, wn, sq);
+    if (i < n_sq) sq = fma(wn, wn, sq);
   }
   sq = block_sum(sq);
   if (threadIdx.x == 0) atomicAdd(&sc->wsq, sq);
@@ -245,8 +247,8 @@ cudaError_t lsqr_launch_init_s1(DevScalars* sc, cudaStream_t st, int64_t* launch
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_sumsq_v(double* v, int64_t n, DevScalars* sc, const double* dinv, cudaStream_t st,
-                                int64_t* launches) {
-  k_sumsq_v<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc, dinv);
+                                int64_t* launches, int64_t n_sq) {
+  k_sumsq_v<<<grid_for(n, 256, 4), 256, 0, st>>>(v, n, sc, dinv, n_sq < 0 ? n : n_sq);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launches) {
@@ -254,8 +256,8 @@ cudaError_t lsqr_launch_init_s2(DevScalars* sc, cudaStream_t st, int64_t* launch
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_init_vw(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
-                                const double* dinv, double* var, cudaStream_t st, int64_t* launches) {
-  k_init_vw<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var);
+                                const double* dinv, double* var, cudaStream_t st, int64_t* launches, int64_t n_sq) {
+  k_init_vw<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var, n_sq < 0 ? n : n_sq);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_t st, int64_t* launches) {
@@ -263,8 +265,8 @@ cudaError_t lsqr_launch_vscale(double* v, int64_t n, DevScalars* sc, cudaStream_
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_vcombine(double* v, const double* g, int64_t n, DevScalars* sc, const double* dinv,
-                                 cudaStream_t st, int64_t* launches) {
-  k_vcombine<<<grid_for(n, 256, 4), 256, 0, st>>>(v, g, n, sc, dinv);
+                                 cudaStream_t st, int64_t* launches, int64_t n_sq) {
+  k_vcombine<<<grid_for(n, 256, 4), 256, 0, st>>>(v, g, n, sc, dinv, n_sq < 0 ? n : n_sq);
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol, double btol, double conlim,
@@ -273,8 +275,8 @@ cudaError_t lsqr_launch_step_scalars(DevScalars* sc, int64_t itnlim, double atol
   return LAUNCHED();
 }
 cudaError_t lsqr_launch_update(double* v, double* w, double* x, int64_t n, DevScalars* sc, double* vs,
-                               const double* dinv, double* var, cudaStream_t st, int64_t* launches) {
-  k_update<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var);
+                               const double* dinv, double* var, cudaStream_t st, int64_t* launches, int64_t n_sq) {
+  k_update<<<grid_for(n, 256, 4), 256, 0, st>>>(v, w, x, n, sc, vs, dinv, var, n_sq < 0 ? n : n_sq);
   return LAUNCHED();
 }
 
@@ -354,6 +356,35 @@ cudaError_t lsqr_launch_scale_by(double* dst, const double* src, const double* s
 }
 cudaError_t lsqr_launch_export_u(const double* uhat, double* u, int64_t M, const DevScalars* sc, cudaStream_t st, int64_t* launches) {
   k_export_u<<<grid_for(M, 256, 4), 256, 0, st>>>(uhat, u, M, sc);
+  return LAUNCHED();
+}
+
+// ---- row-sharded solve (gsr.h gsr_shard_*) --------------------------
+// Between two phases of a sharded solve the caller sums the exchange buffer over the ranks.  This kernel moves the
+// replicated tail of an n-vector (attitude, instrumental, global: ns doubles from `vec`) and the partial sums of
+// squares between the library's own state and that buffer.  No-op once the solve has stopped.
+//   pack   : xbuf[0..ns) = vec (when ns > 0) ; then the scalars named by `what`, appended after the vector part
+//   unpack : the reverse
+__global__ void __launch_bounds__(256) k_shard_xfer(double* __restrict__ vec, int64_t ns, DevScalars* sc,
+                                                    double* __restrict__ xbuf, int what, int unpack) {
+  if (sc->done) return;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < ns; i += (int64_t)gridDim.x * blockDim.x) {
+    if (unpack) vec[i] = xbuf[i];
+    else xbuf[i] = vec[i];
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    double* q = xbuf + ns;
+    if (what == SHARD_X_USQ) { if (unpack) sc->usq = q[0]; else q[0] = sc->usq; }
+    else if (what == SHARD_X_VSQ) { if (unpack) sc->vsq = q[0]; else q[0] = sc->vsq; }
+    else if (what == SHARD_X_USQ_WSQ) {
+      if (unpack) { sc->usq = q[0]; sc->wsq = q[1]; }
+      else { q[0] = sc->usq; q[1] = sc->wsq; }
+    }
+  }
+}
+cudaError_t lsqr_launch_shard_xfer(double* vec, int64_t ns, DevScalars* sc, double* xbuf, int what, int unpack,
+                                   cudaStream_t st, int64_t* launches) {
+  k_shard_xfer<<<grid_for(ns, 256, 4), 256, 0, st>>>(vec, ns, sc, xbuf, what, unpack);
   return LAUNCHED();
 }
 
