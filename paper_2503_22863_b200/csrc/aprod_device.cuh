@@ -28,6 +28,11 @@ constexpr unsigned FULL = 0xffffffffu;
 // with an L2 evict-last policy on the attitude table: profiles/r01_summary.md section 3)
 __device__ __forceinline__ double ld_nc_na(const double* p) { return __ldg(p); }
 
+#ifdef GSR_HOST_EMULATION
+// (tests/emu: host build of the kernels; an atomic add stands in for the L2 reduction)
+__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add_if_ge(double* p, double v, int a, int b) { if (a >= b) atomicAdd(p, v); }
+#else
 // fp64 reduction at L2, fire and forget.  Explicitly .global: a pointer that was read from a table in
 // shared memory would otherwise compile to a GENERIC atomic (no RED, address-space check per lane).
 __device__ __forceinline__ void red_add(double* p, double v) {
@@ -38,6 +43,7 @@ __device__ __forceinline__ void red_add(double* p, double v) {
 __device__ __forceinline__ void red_add_if_ge(double* p, double v, int a, int b) {
   asm volatile("{\n.reg .pred q;\nsetp.ge.s32 q, %2, %3;\n@q red.global.add.f64 [%0], %1;\n}" ::"l"(p), "d"(v), "r"(a), "r"(b) : "memory");
 }
+#endif
 
 // What a kernel needs to gather from x (aprod 1 side).
 struct GatherCtx {
@@ -198,10 +204,14 @@ struct ScatterCtx {
   int acc_part;             // with ins_tab: columns [0, acc_part) are accumulated in acc_s instead (whatever shared memory is left)
 };
 
+#ifdef GSR_HOST_EMULATION
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) { emu::dmma884(c0, c1, a, b); }
+#else
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
+#endif
 
 // x[5*s + k] += sum_{rows r of star s in this tile} a[r][k] * y[r], k < 5   -- Eq. (3), astrometric block.
 // Rows are sorted by star, so a tile covers the consecutive star ids s0 .. s1.  When s1 - s0 < 8 the sums
@@ -329,7 +339,11 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what);
 // lane l reads word 32 c + l, i.e. always its own bank (a single shared copy cost 5.5 wavefronts per LDS at C4).
 __device__ __forceinline__ void load_ins_tab(uint32_t* tab_s, const InstrAcc& ia, int tab_shift) {
   unsigned smid;
+#ifdef GSR_HOST_EMULATION
+  smid = emu::smid();
+#else
   asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+#endif
   int die = smid < (unsigned)SMID_SLOTS ? ia.sm_die[smid] : 0;
   if (die < 0 || !ia.two_dies) die = 0;
   const int set = die * ia.copies_per_die + (int)(blockIdx.x % (unsigned)ia.copies_per_die);

@@ -149,6 +149,10 @@ static int build_att_buffers(gsr_system* s) {
 // block then classifies its share of the pool the same way.  A wrong call only costs speed, never
 // correctness: every chunk is a valid accumulator whoever reduces into it.
 constexpr int N_REF = 16;
+#ifdef GSR_HOST_EMULATION
+// (tests/emu: no dies on the host; every chunk answers alike, so the probe reports one die)
+__device__ __forceinline__ float atom_latency(double* p, int reps) { atomicAdd(p, 0.0); return 100.0f + 0.0f * (float)reps; }
+#else
 __device__ __forceinline__ float atom_latency(double* p, int reps) {
   double v;
   asm volatile("atom.global.add.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "d"(0.0) : "memory");   // warm
@@ -160,10 +164,15 @@ __device__ __forceinline__ float atom_latency(double* p, int reps) {
   const long long t1 = clock64();
   return (float)(t1 - t0) / (float)reps + (float)(v * 0.0);
 }
+#endif
 __global__ void k_probe_homes(double* pool, int n_pool, int* sm_die, signed char* home, int* bimodal) {
   if (threadIdx.x != 0) return;
   unsigned smid;
+#ifdef GSR_HOST_EMULATION
+  smid = emu::smid();
+#else
   asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+#endif
   float ref[N_REF], srt[N_REF];
   const int off = (int)((blockIdx.x * 4u) % INS_CHUNK);   // own sector of every reference chunk: no same-address contention
   for (int c = 0; c < N_REF; c++) atom_latency(pool + (size_t)c * INS_CHUNK + off, 2);   // untimed pass: TLB, first touch

@@ -28,6 +28,23 @@ constexpr int STAGE_BYTES = COEF_TILE_BYTES + IDX_TILE_BYTES;  // 7424 (multiple
 __host__ __device__ constexpr int row_off(int r) { return (r >> 1) * PAIR_BYTES + (r & 1) * 192; }
 __host__ __device__ constexpr int pad_off(int r) { return (r >> 1) * PAIR_BYTES + 384 + (r & 1) * 8; }
 
+#ifdef GSR_HOST_EMULATION
+// tests/emu: the same helpers for the host build of the kernels (test infrastructure; never part of libgsr.so).
+// The copies complete at issue time, so the mbarrier calls reduce to a warp barrier on the waiting side.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(reinterpret_cast<uintptr_t>(p)); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int) { *bar = 0; }
+__device__ __forceinline__ void mbar_fence_init() {}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t*, uint32_t) {}
+__device__ __forceinline__ void mbar_wait(uint64_t*, uint32_t) { __syncwarp(); }
+__device__ __forceinline__ void fence_proxy_async() {}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() { return 0; }
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t*, uint64_t) {
+  emu::tensor_load_2d(dst, map, c0, c1);
+}
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t*, uint64_t) {
+  emu::bulk_copy(dst, src, bytes);
+}
+#else
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
@@ -73,6 +90,7 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
       "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
+#endif  // GSR_HOST_EMULATION
 
 // Per-warp ring of `nstages` row tiles.  All 32 lanes call every method; lane 0 talks to the TMA.
 struct TileRing {

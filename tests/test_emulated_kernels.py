@@ -1,0 +1,170 @@
+"""The bodies of the GPU parity tests, run on the HOST EMULATION of the kernels (tests/emu: csrc/*.cu compiled by g++
+against a stand-in CUDA runtime, one OS thread per CUDA thread, libgsr_emu.so).  No GPU needed.
+
+Why: the code paths added in round 2 (the 23-coefficient record, the constraint section, the sharded phases, column
+norms with repeated columns, the partial shared-memory accumulators) and the GPU tests written for them could not run
+on hardware in that round.  Here the SAME test functions run against the SAME kernel source and the CPU oracle, so a
+logic error in a kernel, in the C ABI or in a test shows up before the GPU run -- and the emulation itself is
+checked by the tests that did pass on hardware in round 1 (they pass here too).  What this cannot show is anything
+about the hardware (timing, the async proxy, the real TMA / tensor-core units); the GPU tests remain the parity
+tests proper.  The emulated library is test infrastructure: the product never loads it and has no CPU fallback.
+
+Default: a subset that runs in about two minutes on 8 cores.  GSR_EMU_FULL=1 runs every GPU test body that fits the host
+(all but the full-size C2...C5 systems, which are dry-run on small stand-in shapes).
+"""
+import importlib
+import os
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, os.path.join(HERE, "emu"))
+
+import harness  # noqa: E402
+from gaia_synth.configs import C4, C5  # noqa: E402
+
+FULL = os.environ.get("GSR_EMU_FULL", "0") == "1"
+pytestmark = pytest.mark.timeout(1800)          # (a rendezvous that never completes must not hang the suite)
+
+# (module, function, args, in the default subset?)
+CASES = [
+    # ---- passed on hardware in round 1: these validate the emulation (and guard the shared code against round 2's edits)
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (1, 1), True),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (1, 31), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (1, 33), True),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (3, 11), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (7, 37), True),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (5, 129), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (2, 1000), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (64, 64), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (300, 1), True),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (150, 3), False),
+    ("test_gpu_parity", "test_aprod_ragged_sizes", (41, 5), True),
+    ("test_gpu_parity", "test_aprod_c1", (), False),
+    ("test_gpu_parity", "test_aprod_skewed_stars_and_hot_knots", (), False),
+    ("test_gpu_parity", "test_aprod_constraint_rows", (), False),
+    ("test_gpu_parity", "test_aprod_n_glob_zero_and_edges", (), True),
+    ("test_gpu_parity", "test_aprod_accumulates", (), False),
+    ("test_gpu_parity", "test_die_local_instrumental_accumulators", (), False),
+    # (test_empty_system_and_errors is not here: its last check is that the binding refuses host tensors)
+    ("test_gpu_parity", "test_lsqr_c1_to_convergence", (), False),
+    ("test_gpu_parity", "test_lsqr_same_iteration_count_early_and_replays", (), False),
+    ("test_gpu_parity", "test_lsqr_stop_codes", (), True),
+    ("test_gpu_parity", "test_lsqr_constraint_rows_to_convergence", (), False),
+    ("test_gpu_parity", "test_lsqr_host_entry_matches_device_entry", (), False),
+    ("test_gpu_precond", "test_variances_plain_lsqr", (), False),
+    ("test_gpu_precond", "test_covariances_of_pairs", (), False),
+    # ---- written or changed in round 2, never run on hardware
+    ("test_gpu_precond", "test_colnorms", ("tiny-noglob",), True),
+    ("test_gpu_precond", "test_colnorms", ("C1",), False),
+    ("test_gpu_precond", "test_colnorms", ("C5-small",), True),
+    ("test_gpu_precond", "test_preconditioned_solve", ("*",), False),
+    ("test_gpu_z_f3", "test_coeff23_products", (1, 1), True),
+    ("test_gpu_z_f3", "test_coeff23_products", (1, 33), True),
+    ("test_gpu_z_f3", "test_coeff23_products", (3, 11), False),
+    ("test_gpu_z_f3", "test_coeff23_products", (7, 37), True),
+    ("test_gpu_z_f3", "test_coeff23_products", (64, 64), False),
+    ("test_gpu_z_f3", "test_coeff23_products", (40, 100), False),
+    ("test_gpu_z_f3", "test_coeff23_lsqr", (), False),
+    ("test_gpu_z_f3", "test_constraint_section_24", (1,), False),
+    ("test_gpu_z_f3", "test_constraint_section_24", (0,), False),
+    ("test_gpu_z_f3", "test_constraint_section_coeff23", (), False),
+    ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (1, 300), False),
+    ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (2, 300), False),
+    ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (3, 300), False),
+    ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (2, 60_000), False),
+    ("test_gpu_zz_sharded", "test_sharded_equals_unsharded_and_state_rules", (), True),
+]
+
+
+def _param_values(mod, fn_name, key):
+    """The parametrize values of a test function whose ids are names ('tiny-noglob', ...), '*' = all of them."""
+    fn = getattr(mod, fn_name)
+    for mark in getattr(fn, "pytestmark", []):
+        if mark.name == "parametrize":
+            values, ids = mark.args[1], mark.kwargs.get("ids")
+            if key == "*":
+                return [(v,) for v in values]
+            if ids and key in ids:
+                return [(values[ids.index(key)],)]
+    raise KeyError(f"{fn_name}: no parametrize id {key!r}")
+
+
+@pytest.mark.parametrize("modname,fn,args,fast", CASES, ids=[f"{m}.{f}{list(a)}" for m, f, a, _ in CASES])
+def test_gpu_test_body_on_host_emulation(modname, fn, args, fast):
+    if not (fast or FULL):
+        pytest.skip("GSR_EMU_FULL=1 runs it")
+    mod = importlib.import_module(modname)
+    gpu_helpers = importlib.import_module("gpu_helpers")
+    calls = [args]
+    if len(args) == 1 and isinstance(args[0], str):
+        calls = _param_values(mod, fn, args[0])
+    with harness.emulated(mod, gpu_helpers):
+        for a in calls:
+            getattr(mod, fn)(*a)
+
+
+# ---- the full-size test bodies, dry-run on small stand-in shapes (their logic, not their size)
+def test_xl_oracle_test_bodies_on_small_shapes():
+    X = importlib.import_module("test_gpu_xl_oracle")
+    gpu_helpers = importlib.import_module("gpu_helpers")
+    saved = (X.SLICE_CASE, X.REPLAY_SHAPE, X.c5_shape)
+    try:
+        with harness.emulated(X, gpu_helpers), harness.fake_cuda_queries():
+            X.SLICE_CASE = (C4.scaled(300, n_knots=500, n_instr=60_000, name="C4-small"), 10_037, 5_011, 1000)
+            X.test_c4_slice_aprod_against_streamed_oracle()          # starts inside a star, ends on a ragged tile
+            X.REPLAY_SHAPE = C4.scaled(120, n_knots=300, n_instr=60_000, name="C4-small")
+            X.test_c4_lsqr_replays_against_oracle()
+            X.c5_shape = lambda: C5.scaled(100, n_knots=150, n_instr=60, n_constraint_rows=20, name="C5-tiny")
+            X.test_c5_to_convergence_against_oracle()
+    finally:
+        X.SLICE_CASE, X.REPLAY_SHAPE, X.c5_shape = saved
+
+
+def test_partial_shared_memory_accumulators_and_private_table():
+    """Options that are off by default because they were never timed in their committed form (acc_part, acc_part_fused:
+    the PART = true kernel instances; tab_private): parity against the oracle at I = 60,000, rows that hit both sides
+    of the split and repeat a column."""
+    P = importlib.import_module("test_gpu_parity")
+    gpu_helpers = importlib.import_module("gpu_helpers")
+    oracle = importlib.import_module("oracle")
+    from gaia_synth import host
+    from helpers import rhs
+    with harness.emulated(P, gpu_helpers):
+        shape = C5.scaled(120, n_knots=400, n_instr=60_000, n_constraint_rows=30)
+        a, idx = host.make_rows(shape)
+        idx[::5, 2:8] = np.array([3, 3, 59_999, 17, 3, 40_000], dtype=np.int32)
+        with P.make_gpu_system(shape, a, idx) as s:
+            for opt in (("acc_part", -1), ("acc_part", 1000), ("tab_private", 1)):
+                s.set_option(*opt)
+                P.check_aprod2(shape, a, idx, s, seed=31)
+                P.check_aprod2(shape, a, idx, s, seed=41)             # the accumulators were flushed and cleared
+            ref = oracle.colnorms(oracle.layout_of(shape), a, idx)     # the square = 1 pass through the same kernels
+            got = s.colnorms(torch.empty(s.n_unknowns, dtype=torch.float64)).numpy()
+            nz = ref > 0
+            assert np.all(got[~nz] == 0.0) and np.max(np.abs(got[nz] - ref[nz]) / ref[nz]) <= 1e-12
+            s.set_option("tab_private", 0)
+            b = rhs(shape, a, idx, host.x_true(shape))
+            for opt in (("acc_part_fused", -1), ("acc_part_fused", 777), ("tab_private", 1)):
+                s.set_option(*opt)
+                s.lsqr_init(P.dev(b))
+                for k in (0, 2):
+                    s.lsqr_iterate(k)
+                    P.replay_one_step(shape, a, idx, s)
+
+
+def test_product_does_not_know_the_emulation():
+    """The emulated library is reachable from tests/ only: nothing under the package, bench.py or __graft_entry__.py
+    names it, and outside a test the binding loads libgsr.so."""
+    root = os.path.dirname(HERE)
+    files = [os.path.join(root, "bench.py"), os.path.join(root, "__graft_entry__.py")]
+    pkg = os.path.join(root, "paper_2503_22863_b200")
+    files += [os.path.join(pkg, f) for f in os.listdir(pkg) if f.endswith(".py")]
+    for p in files:
+        text = open(p).read()
+        assert "libgsr_emu" not in text and "tests/emu" not in text and "build_emu" not in text, p
+    from paper_2503_22863_b200 import binding
+    assert binding._lib is None or "libgsr_emu" not in str(getattr(binding._lib, "_name", ""))
