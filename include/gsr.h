@@ -46,7 +46,8 @@
  *
  * DETERMINISM.  aprod2 uses fp64 reductions at L2 (red.global.add.f64) for the attitude block;
  * the order of those additions varies run to run, so results are reproducible to rounding
- * (normwise ~1e-15), not bit for bit.  aprod1 is bit-reproducible.
+ * (normwise ~1e-15), not bit for bit.  aprod1 is bit-reproducible.  For debugging, option
+ * aprod2_variant = 2 selects a slow aprod2 whose summation order is fixed (gsr_set_option below).
  */
 #ifndef GSR_H
 #define GSR_H
@@ -257,7 +258,14 @@ int gsr_shard_poll(gsr_system *sys, int32_t *stopped, gsr_lsqr_result *res, void
  *                      gather_smem       1 (default) stage the instrumental slice of x in shared memory when it fits
  *                      instr_copies      1 (default) use the replicated accumulators, 0 reduce straight into x
  *                      fused             1 (default) one pass over A per LSQR iteration, 0 aprod 1 then aprod 2
- *                      aprod1_variant, aprod2_variant   1 (default) TMA tiles, 0 one thread per row (cross-check)
+ *                      aprod1_variant, aprod2_variant   1 (default) TMA tiles, 0 one thread per row (cross-check);
+ *                                        aprod2_variant = 2: DETERMINISTIC debug variant -- every sum of gsr_aprod2 (and of the
+ *                                        aprod 2 inside gsr_lsqr_init and the two-pass schedule) has one fixed order that
+ *                                        depends on the sizes only, so results are bit-reproducible run to run and GPU to GPU;
+ *                                        slow by design (at most 1024 threads add up the shared columns), either record format
+ *                      det_chunks        variant 2: row chunks, each with a private copy of the shared columns (0 = default: as
+ *                                        many as fit 256 MB, at most 1024); 1 = row by row, slot by slot from x's initial value,
+ *                                        i.e. Eq. (3) written out as a plain loop: bit-identical to such a serial implementation
  *                      graph             1 (default) small, launch-bound systems (matrix <= 256 MB): the launches of a batch
  *                                        of LSQR iterations are captured once into a CUDA graph and replayed, 0 never
  *                      check_every       LSQR iterations between host polls of the stop flag (default 16)      */

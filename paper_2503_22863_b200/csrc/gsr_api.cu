@@ -321,7 +321,7 @@ extern "C" void gsr_destroy(gsr_system* s) {
   if (!s) return;
   free_iter_graph(s);
   cudaFree(s->u); cudaFree(s->vv); cudaFree(s->w); cudaFree(s->x); cudaFree(s->sc);
-  cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins.pool); cudaFree(s->side.ins.sm_die); cudaFree(s->side.ins.chunk_tab); cudaFree(s->g);
+  cudaFree(s->side.att_il); cudaFree(s->side.att_acc); cudaFree(s->side.ins.pool); cudaFree(s->side.ins.sm_die); cudaFree(s->side.ins.chunk_tab); cudaFree(s->g); cudaFree(s->side.det_part);
   cudaFree(s->dinv); cudaFree(s->vs); cudaFree(s->var);
   free_events(s);
   delete s;
@@ -398,11 +398,40 @@ static int do_aprod1(gsr_system* s, const double* x, bool x_il, double* y, const
   if (e != cudaSuccess) return cuda_fail(e, "aprod1 launch");
   return GSR_OK;
 }
+// deterministic debug variant: how many row chunks (each with a private copy of the shared columns), from the sizes alone
+static int det_chunk_count(const gsr_system* s) {
+  if (s->tune.det_chunks > 0) return s->tune.det_chunks;
+  const int64_t ns = s->v.n - s->v.oA;
+  int64_t c = (int64_t)(256u << 20) / (ns * 8);
+  return (int)(c < 1 ? 1 : (c > 1024 ? 1024 : c));
+}
+static int ensure_det_pool(gsr_system* s, int C) {
+  if (s->side.det_part && s->side.det_cap >= C) return GSR_OK;
+  cudaFree(s->side.det_part);
+  s->side.det_part = nullptr; s->side.det_cap = 0;
+  ALLOC(s->side.det_part, (size_t)C * (size_t)(s->v.n - s->v.oA) * sizeof(double));
+  s->side.det_cap = C;
+  return GSR_OK;
+}
+
 static int do_aprod2(gsr_system* s, const double* y, double* x, bool x_il, const double* yscale, const int* done,
                      cudaStream_t st) {
   EventPair ep;
+  cudaError_t e;
+  if (s->tune.aprod2_variant == 2) {      // deterministic debug variant, both record formats, both sections in row order
+    const int C = det_chunk_count(s);
+    int rc = ensure_det_pool(s, C);
+    if (rc) return rc;
+    const bool p = prof_begin(s, 2, st, &ep);
+    e = launch_aprod2_det(s->v, s->side.det_part, C, s->num_sms, y, x, x_il, yscale, done, st, &s->launches);
+    if (e == cudaSuccess && s->has_con)
+      e = launch_aprod2_det(s->con, s->side.det_part, C, s->num_sms, y + s->v.M, x, x_il, yscale, done, st, &s->launches);
+    if (p) prof_end(s, st, &ep);
+    if (e != cudaSuccess) return cuda_fail(e, "aprod2 (deterministic) launch");
+    return GSR_OK;
+  }
   const bool p = prof_begin(s, 2, st, &ep);
-  cudaError_t e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, x_il, yscale, done, st, &s->launches);
+  e = launch_aprod2(s->v, s->side, s->tune, s->num_sms, y, x, x_il, yscale, done, st, &s->launches);
   if (e == cudaSuccess && s->has_con)
     e = launch_aprod2(s->con, s->con_side, s->tune, s->num_sms, y + s->v.M, x, x_il, yscale, done, st, &s->launches);
   if (p) prof_end(s, st, &ep);
@@ -542,7 +571,7 @@ struct IterGraph {
   int64_t n_iters = 0, itnlim = 0, launches = 0, n_cov = 0;
   double atol = 0, btol = 0, conlim = 0;
   int fused = 0, warps = 0, stages = 0, acc_smem = 0, gather_smem = 0, die_local = 0, instr_copies = 0, ctas = 0;
-  int a1v = 0, a2v = 0, tabp = 0, accp = 0, accpf = 0;
+  int a1v = 0, a2v = 0, tabp = 0, accp = 0, accpf = 0, detc = 0;
   bool precond = false, var = false, cov = false;
   const void *j1 = nullptr, *j2 = nullptr, *covp = nullptr;
 };
@@ -550,7 +579,7 @@ static bool same_key(const IterGraph& a, const IterGraph& b) {
   return a.n_iters == b.n_iters && a.itnlim == b.itnlim && a.atol == b.atol && a.btol == b.btol && a.conlim == b.conlim &&
          a.fused == b.fused && a.warps == b.warps && a.stages == b.stages && a.acc_smem == b.acc_smem &&
          a.gather_smem == b.gather_smem && a.die_local == b.die_local && a.instr_copies == b.instr_copies &&
-         a.ctas == b.ctas && a.a1v == b.a1v && a.a2v == b.a2v && a.tabp == b.tabp && a.accp == b.accp && a.accpf == b.accpf && a.precond == b.precond && a.var == b.var &&
+         a.ctas == b.ctas && a.a1v == b.a1v && a.a2v == b.a2v && a.tabp == b.tabp && a.accp == b.accp && a.accpf == b.accpf && a.detc == b.detc && a.precond == b.precond && a.var == b.var &&
          a.cov == b.cov && a.n_cov == b.n_cov && a.j1 == b.j1 && a.j2 == b.j2 && a.covp == b.covp;
 }
 
@@ -581,7 +610,7 @@ extern "C" int gsr_lsqr_iterate(gsr_system* s, int64_t n_iters, int64_t itnlim, 
   key.n_iters = n_iters; key.itnlim = itnlim; key.atol = atol; key.btol = btol; key.conlim = conlim;
   key.fused = s->tune.fused; key.warps = s->tune.warps; key.stages = s->tune.stages; key.acc_smem = s->tune.acc_smem;
   key.gather_smem = s->tune.gather_smem; key.die_local = s->tune.die_local; key.instr_copies = s->tune.instr_copies;
-  key.ctas = s->tune.ctas_per_sm; key.a1v = s->tune.aprod1_variant; key.a2v = s->tune.aprod2_variant; key.tabp = s->tune.tab_private; key.accp = s->tune.acc_part; key.accpf = s->tune.acc_part_fused;
+  key.ctas = s->tune.ctas_per_sm; key.a1v = s->tune.aprod1_variant; key.a2v = s->tune.aprod2_variant; key.tabp = s->tune.tab_private; key.accp = s->tune.acc_part; key.accpf = s->tune.acc_part_fused; key.detc = s->tune.det_chunks;
   key.precond = s->opt_precond; key.var = s->opt_var; key.cov = s->opt_cov; key.n_cov = s->n_cov;
   key.j1 = s->cov_j1; key.j2 = s->cov_j2; key.covp = s->cov;
   IterGraph* g = s->iter_graph;
@@ -990,6 +1019,7 @@ extern "C" int gsr_set_option(gsr_system* s, const char* name, int64_t value) {
   else if (!strcmp(name, "die_local")) s->tune.die_local = (int)value;
   else if (!strcmp(name, "graph")) s->tune.graph = (int)value;
   else if (!strcmp(name, "gather_smem")) s->tune.gather_smem = (int)value;
+  else if (!strcmp(name, "det_chunks")) { if (value < 0 || value > 65536) return GSR_EINVAL; s->tune.det_chunks = (int)value; }
   else if (!strcmp(name, "tab_private")) s->tune.tab_private = (int)value;
   else if (!strcmp(name, "acc_part")) s->tune.acc_part = (int)value;
   else if (!strcmp(name, "acc_part_fused")) s->tune.acc_part_fused = (int)value;

@@ -37,7 +37,10 @@ struct DevScalars {
 
 struct Tuning {
   int aprod1_variant = 1;  // 1 = TMA-staged tiles (default), 0 = one thread per row (simple)
-  int aprod2_variant = 1;  // 1 = TMA-staged tiles, split by parameter block (default), 0 = one thread per row
+  int aprod2_variant = 1;  // 1 = TMA-staged tiles, split by parameter block (default), 0 = one thread per row,
+                           // 2 = deterministic debug variant (aprod2_det.cu): fixed summation order, bit-reproducible
+  int det_chunks = 0;      // variant 2: row chunks with a private copy of the shared columns each (0 = as many as fit 256 MB,
+                           // at most 1024; 1 = Eq. (3) as a plain loop: row by row, slot by slot)
   int ctas_per_sm = 0;     // 0 = default of the variant
   int warps = 0;           // warps per CTA of the TMA kernels (0 = the planner's choice: 12, down to 8 if that lets the tables fit)
   int stages = 0;          // ring depth per warp (0 = default 2)
@@ -85,6 +88,8 @@ struct SideData {
   double* att_il = nullptr;   // 3K: interleaved copy of x's attitude block (standalone aprod 1)
   double* att_acc = nullptr;  // 3K: interleaved attitude accumulator, zero between calls (standalone aprod 2)
   InstrAcc ins;               // die-local replicated instrumental accumulators (global memory, L2-resident)
+  double* det_part = nullptr; // aprod2 variant 2: det_cap private copies of the shared columns (allocated on first use)
+  int det_cap = 0;
 };
 
 #ifndef GSR_MAX_TMA_WARPS
@@ -103,6 +108,9 @@ cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t,
 cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* y,
                           double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
                           int64_t* launches, int square = 0);
+//   aprod2, deterministic debug variant (aprod2_det.cu): C chunks of rows, det_part = C * (n - 5S) doubles of scratch
+cudaError_t launch_aprod2_det(const SysView& s, double* det_part, int C, int num_sms, const double* y, double* x, bool x_il,
+                              const double* yscale, const int* done, cudaStream_t st, int64_t* launches);
 cudaError_t launch_validate(const SysView& s, int* flag, cudaStream_t st, int64_t* launches);
 //   fused LSQR step: uh <- A v + c0 uh ; g += A^T uh ; usq += ||uh||^2   (lsqr_fused.cu; v, g internal layout)
 cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning& t, int num_sms, const double* v,

@@ -86,6 +86,8 @@ static inline double atomicAdd(double* p, double v) {
 static inline int atomicAdd(int* p, int v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
 static inline int atomicOr(int* p, int v) { return __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
 static inline int atomicAnd(int* p, int v) { return __atomic_fetch_and(p, v, __ATOMIC_RELAXED); }
+static inline double __dmul_rn(double a, double b) { return a * b; }   // (built with -ffp-contract=off)
+static inline double __dadd_rn(double a, double b) { return a + b; }
 using std::fma;
 using std::sqrt;
 using std::fabs;

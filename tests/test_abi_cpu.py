@@ -88,7 +88,7 @@ def test_no_cpu_fallback():
     with pytest.raises(TypeError):
         gsr.gsr_create(1, 8, 6, 1, torch.zeros((4, 24), dtype=torch.float64), torch.zeros((4, 8), dtype=torch.int32))
     src = "".join(open(os.path.join(ROOT, "paper_2503_22863_b200", f)).read()
-                  for f in ("__init__.py", "binding.py", "build.py"))
+                  for f in ("__init__.py", "binding.py", "build.py", "sharded.py"))
     assert "import oracle" not in src and "from oracle" not in src
     for f in os.listdir(os.path.join(ROOT, "paper_2503_22863_b200", "csrc")):
         assert "oracle" not in open(os.path.join(ROOT, "paper_2503_22863_b200", "csrc", f)).read().lower()

@@ -77,6 +77,12 @@ CASES = [
     ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (3, 300), False),
     ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (2, 60_000), False),
     ("test_gpu_zz_sharded", "test_sharded_equals_unsharded_and_state_rules", (), True),
+    ("test_gpu_zzz_deterministic", "test_deterministic_aprod2", (1, 1), True),
+    ("test_gpu_zzz_deterministic", "test_deterministic_aprod2", (7, 37), True),
+    ("test_gpu_zzz_deterministic", "test_deterministic_aprod2", (64, 64), False),
+    ("test_gpu_zzz_deterministic", "test_deterministic_aprod2", (300, 1), False),
+    ("test_gpu_zzz_deterministic", "test_deterministic_aprod2_skewed_stars_and_sections", (), True),
+    ("test_gpu_zzz_deterministic", "test_lsqr_two_pass_with_deterministic_aprod2", (), True),
 ]
 
 
