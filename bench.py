@@ -51,6 +51,9 @@ def parse():
                     help="uniform-starts: the workload with uniform attitude starts instead of its hot-knot mixture")
     ap.add_argument("--mode", default="iterate", choices=["iterate", "extras"],
                     help="extras: time gsr_colnorms / gsr_lsqr_ex (preconditioned, variances) / covariance pairs")
+    ap.add_argument("--coeff23", action="store_true",
+                    help="control: the same workload with N_Glob = 0 in the 23-coefficient production record (184-byte rows, "
+                         "GSR_LAYOUT_COEFF23) instead of the padded 24-slot record")
     ap.add_argument("--reps", type=int, default=20, help="repetitions of the single aprod 1 / aprod 2 timings")
     ap.add_argument("--cov-pairs", type=int, action="append", default=[], help="--mode extras: pair counts to time")
     return ap.parse_args()
@@ -128,11 +131,13 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def algorithmic_bytes(m, n):
-    """SURVEY.md section 8(d) / DESIGN.md section 7: fixed formulas."""
-    return {"aprod1": 240 * m + 8 * n, "aprod2": 232 * m + 16 * n, "iteration": 472 * m + 96 * n,
+def algorithmic_bytes(m, n, cpr=24):
+    """SURVEY.md section 8(d) / DESIGN.md section 7: fixed formulas (192-byte records; with --coeff23 the record is
+    8 * 23 = 184 bytes and the formulas shrink by 8 bytes per row and pass)."""
+    rec = 8 * cpr + 32
+    return {"aprod1": (rec + 16) * m + 8 * n, "aprod2": (rec + 8) * m + 16 * n, "iteration": (2 * rec + 24) * m + 96 * n,
             # fused LSQR pass: coefficients + indices once, u read + write, v gathered, g read-modify-written
-            "lsqr_fused": 240 * m + 24 * n}
+            "lsqr_fused": (rec + 16) * m + 24 * n}
 
 
 def measured_peak():
@@ -307,9 +312,26 @@ def run_gsr(args):
     if args.mode == "extras":
         return run_extras(args, shape, dev, rank, world)
 
-    vals, idx = gdev.make_system(shape, device=dev)
+    cpr = 24
+    if args.coeff23:
+        # the production record: N_Glob = 0, 23 doubles per row.  Generated block by block (the 24-slot rows of a block,
+        # slots 0..22 packed) so that C4 never holds both storages.
+        from dataclasses import replace
+        shape = replace(shape, n_glob=0, name=shape.name + "[N_Glob = 0, 23-coefficient record]")
+        cpr = 23
+        m_all = shape_rows(shape)
+        vals = torch.empty((m_all, 23), dtype=torch.float64, device=dev)
+        idx = torch.empty((m_all, 8), dtype=torch.int32, device=dev)
+        blk = 8_000_000
+        for r0 in range(0, m_all, blk):
+            v24, i24 = gdev.make_system(shape, device=dev, r0=r0, r1=min(r0 + blk, m_all))
+            vals[r0:r0 + v24.shape[0]].copy_(v24[:, :23])
+            idx[r0:r0 + v24.shape[0]].copy_(i24)
+            del v24, i24
+    else:
+        vals, idx = gdev.make_system(shape, device=dev)
     m, n = int(vals.shape[0]), shape.n_unknowns
-    sysm = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx)
+    sysm = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx, coeffs_per_row=cpr)
     for opt in args.option:
         k, v = opt.split("=")
         sysm.set_option(k, int(v))
@@ -382,7 +404,7 @@ def run_gsr(args):
     ap2_alone = median_ms(lambda: sysm.aprod2(yv, xv))
     del xv, yv
 
-    ab = algorithmic_bytes(m, n)
+    ab = algorithmic_bytes(m, n, cpr)
     peak, peak_src = measured_peak()
     cands = [("aprod1", ap1_ms, ap1_n), ("aprod2", ap2_ms, ap2_n), ("lsqr_fused", fu_ms, fu_n)]
     dom, dom_ms, dom_n = max(cands, key=lambda c: c[1] * c[2])
@@ -412,7 +434,7 @@ def run_gsr(args):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{shape.name}: {m} rows x {n} unknowns (S={shape.n_stars}, K={shape.n_knots}/axis, "
                                    f"I={shape.n_instr}, G={shape.n_glob})",
-                       "matrix_bytes": m * 224, "l2_policy": "inputs (matrix) far larger than L2; no flush",
+                       "matrix_bytes": m * (8 * cpr + 32), "coeffs_per_row": cpr, "l2_policy": "inputs (matrix) far larger than L2; no flush",
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                        "timed_path": "CUDA-graph replay, profiling off" if graph_path else "eager launches, per-kernel events on",
                        "options": args.option},
@@ -435,7 +457,7 @@ def run_gsr(args):
 
     # ---- CPU baseline: the oracle, as it stands, on a bounded sample (rank 0, N = 1 only).  A failure of this leg or
     # of the end-to-end leg (host memory, say) is reported in the line instead of losing the device-timed result.
-    if rank == 0 and world == 1 and not args.no_cpu:
+    if rank == 0 and world == 1 and not args.no_cpu and cpr == 24:
         try:
             ms_rows = oracle_sample_rows(m, args.oracle_rows)
             a_h = vals[:ms_rows].cpu().numpy()
@@ -447,7 +469,7 @@ def run_gsr(args):
                                     "sample": f"failed: {type(ex).__name__}: {ex}"}
 
     # ---- end to end: the C-ABI call with HOST buffers (H2D of the system + K iterations + D2H of x)
-    if not args.no_e2e:
+    if not args.no_e2e and cpr == 24:
         try:
             line["e2e"] = run_e2e(args, shape, sysm, vals, idx, b, m, n, K, dev, rank)
         except Exception as ex:                                    # noqa: BLE001

@@ -80,9 +80,9 @@ typedef struct {
 #define GSR_LAYOUT_TRUSTED 1
 #define GSR_LAYOUT_COEFF23 2 /* values records hold 23 doubles (184 B): the production record without the global
                                 slot (N_Glob = 0; requires n_glob = 0).  Slots keep their numbers.
-                                First version: served by the one-thread-per-row kernels and the two-pass LSQR
-                                schedule (184-byte rows have no 16-byte alignment and no whole-line row-pair TMA
-                                view); gsr_lsqr_ex with GSR_PRECOND_COLNORM returns GSR_ESTATE for it.             */
+                                Served by the same tile kernels through a tensor view of 4-row groups (4 x 184 B = 736 B
+                                is a whole number of 16-byte units); every call of this header
+                                works for it, the fused LSQR pass and column-norm preconditioning included.             */
 
 typedef struct {
   int32_t istop; /* Paige-Saunders stop code 0..7 (not an error)                      */
@@ -224,7 +224,7 @@ int gsr_lsqr_ex(gsr_system *sys, const double *b, double *x, double *var, int32_
  *                     NULL) as gsr_lsqr.  Synchronises `stream`.  The solution is read with gsr_lsqr_result_get: the
  *                     astrometric block holds this rank's stars (0 elsewhere: the sum over ranks is the whole block),
  *                     the other blocks are identical on every rank.
- * Plain LSQR on the one-pass schedule only (GSR_ESTATE with option fused=0 or GSR_LAYOUT_COEFF23); gsr_lsqr_iterate
+ * Plain LSQR on the one-pass schedule only (GSR_ESTATE with option fused=0); gsr_lsqr_iterate
  * returns GSR_ESTATE while a sharded solve is in progress; gsr_lsqr_init / gsr_lsqr end it.                          */
 #define GSR_SHARD_MORE 0
 #define GSR_SHARD_INIT_DONE 1

@@ -5,7 +5,7 @@
 namespace gsr {
 
 // ---- variant 1 (default): TMA-staged row tiles, one warp per tile ---------------------------------
-template <bool GSMEM>
+template <class REC, bool GSMEM>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ x,
              const double* __restrict__ att_il, double* __restrict__ y, const double* __restrict__ c0p, double* sumsq,
@@ -24,7 +24,7 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * nstages * STAGE_BYTES);
   double* xi_s = reinterpret_cast<double*>(bars + nwarps * nstages + 2);
 
-  TileRing ring;
+  TileRing<REC> ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
   if (GSMEM) {
@@ -48,14 +48,14 @@ k_aprod1_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     }
     char* tile = ring.acquire(t, lane);
     RowRegs row;
-    load_row(tile, lane, valid, row);
+    load_row<REC>(tile, lane, valid, row);
     int ts[16];
     att_starts(tile, al, ts);
     __syncwarp();   // every lane holds its row: the exchange runs may be written
-    att_gather(tile, al, ts, att_il);
+    att_gather<REC>(tile, al, ts, att_il);
     const double rest = row_dot_rest<GSMEM>(row, gc);
     __syncwarp();
-    const double out = fma(c0, yin, att_dot_row(tile, lane, row) + rest);
+    const double out = fma(c0, yin, att_dot_row<REC>(tile, lane, row) + rest);
     if (valid) {
       y[r] = out;
       sq = fma(out, out, sq);
@@ -170,15 +170,15 @@ SmemPlan plan_smem(const SysView& s, const Tuning& t, int what) {
 static cudaError_t launch_tma1(bool gsmem, const SysView& s, const SideData& sd, int grid, const SmemPlan& p,
                                const double* x, const double* att_il, double* y, const double* c0, double* sumsq,
                                int* done, cudaStream_t st) {
-  auto k = gsmem ? k_aprod1_tma<true> : k_aprod1_tma<false>;
+  auto k = s.cpr == NSLOT ? (gsmem ? k_aprod1_tma<Rec24, true> : k_aprod1_tma<Rec24, false>)
+                          : (gsmem ? k_aprod1_tma<Rec23, true> : k_aprod1_tma<Rec23, false>);
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
   if (e != cudaSuccess) return e;
   k<<<grid, p.warps * 32, p.bytes, st>>>(sd.map, s, p.stages, x, att_il, y, c0, sumsq, done);
   return cudaGetLastError();
 }
 
-// ---- variant 0: one thread per row, direct global loads (simple device-side cross-check; the path of the
-// 23-coefficient record, whose 184-byte rows have no 16-byte alignment and no row-pair TMA view) -----------------
+// ---- variant 0: one thread per row, direct global loads (simple device-side cross-check, either record format) ----
 __global__ void __launch_bounds__(256) k_aprod1_rowthread(SysView s, const double* __restrict__ x, bool x_il,
                                                           double* __restrict__ y,
                                                           const double* __restrict__ c0p,
@@ -232,7 +232,7 @@ cudaError_t launch_aprod1(const SysView& s, const SideData& sd, const Tuning& t,
                           bool x_il, double* y, const double* c0, double* sumsq, int* done, cudaStream_t st,
                           int64_t* launches) {
   if (s.M == 0) return cudaSuccess;
-  if (t.aprod1_variant == 1 && s.cpr == NSLOT) {   // (the TMA row-pair view needs the 192-byte record)
+  if (t.aprod1_variant == 1) {
     const SmemPlan p = plan_smem(s, t, PLAN_APROD1);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const double* att_il = x + s.oA;

@@ -7,7 +7,7 @@ namespace gsr {
 
 // ---- variant 1 (default): TMA-staged row tiles, split by parameter block (aprod_device.cuh) ------
 // PART: see lsqr_fused.cu
-template <bool ASMEM, bool PART>
+template <class REC, bool ASMEM, bool PART>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ y,
              double* __restrict__ x, double* __restrict__ gatt_il, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
@@ -22,7 +22,7 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   if (!PART) acc_part = 0;
   uint32_t* tab_s = reinterpret_cast<uint32_t*>(acc_s + (ASMEM ? 0 : ((acc_part + 1) & ~1)));
 
-  TileRing ring;
+  TileRing<REC> ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
   const int64_t n_acc = ASMEM ? s.I : (PART ? acc_part : 0);   // accumulators privatised in shared memory: all, or the leading columns
@@ -48,7 +48,7 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     char* tile = ring.acquire(t, lane);
     RowRegs row;
-    load_row(tile, lane, valid, row);
+    load_row<REC>(tile, lane, valid, row);
     if (square) {
       // squared column norms of A as an operator: a column that repeats inside a row (instrumental slots only)
       // contributes (sum of its coefficients)^2 once -- summed in slot order into the first of its slots
@@ -68,10 +68,10 @@ k_aprod2_tma(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     int ts[16];
     att_starts(tile, al, ts);
     __syncwarp();   // every lane holds its row: the exchange runs may be written
-    att_products(tile, lane, row, yv);
+    att_products<REC>(tile, lane, row, yv);
     __syncwarp();
-    att_scatter(tile, al, ts, gatt_il);
-    astro_scatter(tile, lane, nvalid, valid, row, yv, sc.x, square != 0);
+    att_scatter<REC>(tile, al, ts, gatt_il);
+    astro_scatter<REC>(tile, lane, nvalid, valid, row, yv, sc.x, square != 0);
     gacc += scatter_rest<ASMEM, PART>(row, lane, valid, yv, sc);
     ring.release(lane);
   }
@@ -115,8 +115,7 @@ cudaError_t launch_fold_instr(const SysView& s, const SideData& sd, double* x, c
   return cudaGetLastError();
 }
 
-// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check; the path of the
-// 23-coefficient record).  square = 1: squared column norms (y = 1, coefficients squared; equal columns of a row
+// ---- variant 0: one thread per row, fp64 reductions at L2 for every slot (simple cross-check, either record format).  square = 1: squared column norms (y = 1, coefficients squared; equal columns of a row
 // summed first, reading R22) -----------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_aprod2_rowthread(SysView s, const double* __restrict__ y,
                                                           double* __restrict__ x, bool x_il,
@@ -178,13 +177,15 @@ cudaError_t launch_aprod2(const SysView& s, const SideData& sd, const Tuning& t,
                           double* x, bool x_il, const double* yscale, const int* done, cudaStream_t st,
                           int64_t* launches, int square) {
   if (s.M == 0) return cudaSuccess;
-  if ((t.aprod2_variant == 1 || square) && s.cpr == NSLOT) {   // (the TMA row-pair view needs the 192-byte record)
+  if (t.aprod2_variant == 1 || (square && t.aprod2_variant != 0)) {
     const SmemPlan p = plan_smem(s, t, PLAN_APROD2);
     if (p.bytes > SMEM_BUDGET || p.warps > MAX_TMA_WARPS || p.warps < 1 || p.stages < 1) return cudaErrorInvalidValue;
     const int grid = num_sms * (t.ctas_per_sm > 0 ? t.ctas_per_sm : 1);
     const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
     const bool part = use_copies && p.acc_part > 0;
-    auto k = p.acc_smem ? k_aprod2_tma<true, false> : (part ? k_aprod2_tma<false, true> : k_aprod2_tma<false, false>);
+    auto k = s.cpr == NSLOT
+                 ? (p.acc_smem ? k_aprod2_tma<Rec24, true, false> : (part ? k_aprod2_tma<Rec24, false, true> : k_aprod2_tma<Rec24, false, false>))
+                 : (p.acc_smem ? k_aprod2_tma<Rec23, true, false> : (part ? k_aprod2_tma<Rec23, false, true> : k_aprod2_tma<Rec23, false, false>));
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
     InstrAcc ia = sd.ins;

@@ -1,6 +1,7 @@
 // Per-tile device routines shared by the aprod1, aprod2 and fused LSQR kernels.
-// A tile is 32 rows staged in shared memory by TMA (tma.cuh): coefficients as 16 row pairs with a
-// 400-byte pair stride, then the 32 index records.
+// A tile is 32 rows staged in shared memory by TMA (tma.cuh): coefficients in groups of rows (REC = Rec24: 16 pairs
+// with a 400-byte stride; REC = Rec23: 8 groups of four 184-byte rows with an 800-byte stride), then the 32 index
+// records.  Every routine that touches the staged tile is a template on REC.
 //
 // What bounds these kernels on B200 at C4 is the number of requests that leave the SM per row (one per clock
 // into the crossbar, an fp64 reduction counting ~1.65), not DRAM bytes and not shared-memory
@@ -54,12 +55,13 @@ struct GatherCtx {
   double xg;                // x[oG] (0 when G = 0)
 };
 
-// A staged row: 24 coefficients at row_off(r) of the tile (tma.cuh).  Once the owning lane holds the row
+// A staged row: its coefficients at REC::row_off(r) of the tile (tma.cuh).  Once the owning lane holds the row
 // in registers, bytes [XOFF, XOFF+96) of the record (attitude slots 1-11 + instrumental slot 0) are
-// reused as the row's EXCHANGE RUN: 12 doubles in run order p = 3*j + ax (coefficient slot 5 + 4*ax + j),
-// 16-byte aligned so the owner moves it with 6 conflict-free LDS.128 / STS.128 and the cooperative
-// lanes with one LDS.64 / STS.64 per row.  The 8 bytes at pad_off(r) (zero pad of the TMA box) carry the
-// row's y value for the astrometric matrix product.  Bytes [0, 40) (astro slots) stay intact.
+// reused as the row's EXCHANGE RUN: 12 doubles in run order p = 3*j + ax (coefficient slot 5 + 4*ax + j).
+// Rec24: 16-byte aligned, so the owner moves it with 6 conflict-free LDS.128 / STS.128; Rec23: 8-byte aligned (12
+// LDS.64 / STS.64).  The cooperative lanes use one LDS.64 / STS.64 per row either way.  The 8 bytes at REC::y_off(r)
+// (zero pad of the TMA box) carry the row's y value for the astrometric matrix product.  Bytes [0, 40) (astro
+// slots) stay intact.
 constexpr int XOFF = 48;
 
 // The lane-per-row view of a staged tile in registers: all 24 coefficients + the index record.
@@ -68,17 +70,26 @@ struct RowRegs {
   int4 i0, i1;    // {star, att_start, instr0, instr1}, {instr2..5}
 };
 
-// Lane l reads row l of the tile: conflict-free LDS.128 (row_off, tma.cuh), and the 32-byte index
-// record as two LDS.128 issued in swizzled order (lanes 4-7, 12-15, ... read the second half
+// Lane l reads row l of the tile: conflict-free LDS.128 (Rec24) or LDS.64 (Rec23; slot 23 reads as 0), and the
+// 32-byte index record as two LDS.128 issued in swizzled order (lanes 4-7, 12-15, ... read the second half
 // first), which makes the 32-byte-stride pattern bank-conflict free.
 // Tail lanes (row >= M) get zero coefficients (TMA zero fill) and an all-zero index record.
+template <class REC>
 __device__ __forceinline__ void load_row(const char* tile, int lane, bool valid, RowRegs& r) {
-  const double2* ap = reinterpret_cast<const double2*>(tile + row_off(lane));
+  if (REC::VEC16) {
+    const double2* ap = reinterpret_cast<const double2*>(tile + REC::row_off(lane));
 #pragma unroll
-  for (int q = 0; q < NSLOT / 2; q++) {
-    const double2 c = ap[q];
-    r.a[2 * q] = c.x;
-    r.a[2 * q + 1] = c.y;
+    for (int q = 0; q < NSLOT / 2; q++) {
+      const double2 c = ap[q];
+      r.a[2 * q] = c.x;
+      r.a[2 * q + 1] = c.y;
+    }
+  } else {
+    const double* ap = reinterpret_cast<const double*>(tile + REC::row_off(lane));
+#pragma unroll
+    for (int k = 0; k < REC::CPR; k++) r.a[k] = ap[k];
+#pragma unroll
+    for (int k = REC::CPR; k < NSLOT; k++) r.a[k] = 0.0;
   }
   const int4* ip = reinterpret_cast<const int4*>(tile + COEF_TILE_BYTES + lane * 32);
   const int sw = (lane >> 2) & 1;
@@ -108,6 +119,7 @@ __device__ __forceinline__ void att_starts(const char* tile, const AttLane& L, i
 
 // Gather side: exchange run of row <- x_att(il)[3*t_row .. +12).  16 independent 8-byte loads per lane
 // in flight at once.  Call after every lane has loaded its row (a __syncwarp()).
+template <class REC>
 __device__ __forceinline__ void att_gather(char* tile, const AttLane& L, const int (&t)[16],
                                            const double* __restrict__ att_il) {
   if (L.act) {
@@ -116,19 +128,26 @@ __device__ __forceinline__ void att_gather(char* tile, const AttLane& L, const i
     for (int it = 0; it < 16; it++) v[it] = ld_nc_na(att_il + 3 * (int64_t)t[it] + L.p);
 #pragma unroll
     for (int it = 0; it < 16; it++)
-      *reinterpret_cast<double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p) = v[it];
+      *reinterpret_cast<double*>(tile + REC::coop_off(it, L.h) + XOFF + 8 * L.p) = v[it];
   }
 }
 
 // Owner side: sum_{ax,j} a[r][5+4ax+j] * x_att[ax*K + t_r + j] from the row's exchange run.
+template <class REC>
 __device__ __forceinline__ double att_dot_row(const char* tile, int lane, const RowRegs& r) {
-  const double2* xr = reinterpret_cast<const double2*>(tile + row_off(lane) + XOFF);
   double xv[12];
+  if (REC::VEC16) {
+    const double2* xr = reinterpret_cast<const double2*>(tile + REC::row_off(lane) + XOFF);
 #pragma unroll
-  for (int q = 0; q < 6; q++) {
-    const double2 c = xr[q];
-    xv[2 * q] = c.x;
-    xv[2 * q + 1] = c.y;
+    for (int q = 0; q < 6; q++) {
+      const double2 c = xr[q];
+      xv[2 * q] = c.x;
+      xv[2 * q + 1] = c.y;
+    }
+  } else {
+    const double* xr = reinterpret_cast<const double*>(tile + REC::row_off(lane) + XOFF);
+#pragma unroll
+    for (int q = 0; q < 12; q++) xv[q] = xr[q];
   }
   double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
 #pragma unroll
@@ -142,8 +161,8 @@ __device__ __forceinline__ double att_dot_row(const char* tile, int lane, const 
 
 // Owner side of the scatter: exchange run of the lane's row <- a[r][slot(p)] * y[r]; pad <- y[r].
 // (The lane only overwrites what it alone reads, so no barrier is needed after att_dot_row.)
+template <class REC>
 __device__ __forceinline__ void att_products(char* tile, int lane, const RowRegs& r, double yv) {
-  double2* xr = reinterpret_cast<double2*>(tile + row_off(lane) + XOFF);
   double pr[12];
 #pragma unroll
   for (int j = 0; j < 4; j++) {
@@ -151,21 +170,29 @@ __device__ __forceinline__ void att_products(char* tile, int lane, const RowRegs
     pr[3 * j + 1] = r.a[9 + j] * yv;
     pr[3 * j + 2] = r.a[13 + j] * yv;
   }
+  if (REC::VEC16) {
+    double2* xr = reinterpret_cast<double2*>(tile + REC::row_off(lane) + XOFF);
 #pragma unroll
-  for (int q = 0; q < 6; q++) xr[q] = make_double2(pr[2 * q], pr[2 * q + 1]);
-  *reinterpret_cast<double*>(tile + pad_off(lane)) = yv;
+    for (int q = 0; q < 6; q++) xr[q] = make_double2(pr[2 * q], pr[2 * q + 1]);
+  } else {
+    double* xr = reinterpret_cast<double*>(tile + REC::row_off(lane) + XOFF);
+#pragma unroll
+    for (int q = 0; q < 12; q++) xr[q] = pr[q];
+  }
+  *reinterpret_cast<double*>(tile + REC::y_off(lane)) = yv;
 }
 
 // g_att(il)[3*t_r + p] += a[r][slot(p)] * y[r]  -- PAPER.md:49, Eq. (3), attitude block: per pass one
 // red.global.add.f64 instruction whose 12 active lanes of each half-warp cover one contiguous run.
 // Call after a __syncwarp() that follows att_products.
+template <class REC>
 __device__ __forceinline__ void att_scatter(const char* tile, const AttLane& L, const int (&t)[16],
                                             double* __restrict__ gatt_il) {
   if (L.act) {
 #pragma unroll
     for (int it = 0; it < 16; it++)
       red_add(gatt_il + 3 * (int64_t)t[it] + L.p,
-              *reinterpret_cast<const double*>(tile + it * PAIR_BYTES + L.h * 192 + XOFF + 8 * L.p));
+              *reinterpret_cast<const double*>(tile + REC::coop_off(it, L.h) + XOFF + 8 * L.p));
   }
 }
 
@@ -223,6 +250,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // Otherwise (stars with < 5 rows, or unused star ids inside the tile): 5 reductions per row.
 // Requires: att_products(yv) stored (yv = 0 for rows past the end) and a __syncwarp() since.
 // square: the staged coefficients are squared on the fly (column-norm pass; r.a is squared by the caller).
+template <class REC>
 __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nvalid, bool valid, const RowRegs& r,
                                               double yv, double* __restrict__ x, bool square = false) {
   const int s0 = __shfl_sync(FULL, r.i0.x, 0), s1 = __shfl_sync(FULL, r.i0.x, nvalid - 1);
@@ -233,8 +261,8 @@ __device__ __forceinline__ void astro_scatter(const char* tile, int lane, int nv
     for (int j = 0; j < 8; j++) {
       const int row = 4 * j + i;
       const int st = *reinterpret_cast<const int*>(tile + COEF_TILE_BYTES + row * 32);
-      const double y = *reinterpret_cast<const double*>(tile + pad_off(row));
-      double b = *reinterpret_cast<const double*>(tile + row_off(row) + 8 * (q < 5 ? q : 0));
+      const double y = *reinterpret_cast<const double*>(tile + REC::y_off(row));
+      double b = *reinterpret_cast<const double*>(tile + REC::row_off(row) + 8 * (q < 5 ? q : 0));
       if (square) b *= b;
       if (j & 1) dmma884(d0, d1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);
       else dmma884(c0, c1, (st - s0 == q) ? y : 0.0, q < 5 ? b : 0.0);

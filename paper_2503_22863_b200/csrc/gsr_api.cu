@@ -7,6 +7,7 @@
 #include <vector>
 
 #include "gsr_internal.cuh"
+#include "tma.cuh"
 
 using namespace gsr;
 
@@ -83,8 +84,8 @@ struct gsr_system {
 
 static inline cudaStream_t S(void* s) { return reinterpret_cast<cudaStream_t>(s); }
 static inline int64_t m_total(const gsr_system* s) { return s->v.M + s->con.M; }      // observation + constraint rows
-// one pass over A per LSQR iteration needs the TMA kernels, hence the 192-byte record
-static inline bool fused_path(const gsr_system* s) { return s->tune.fused && s->v.cpr == NSLOT; }
+// one pass over A per LSQR iteration (the TMA tile kernels, either record format)
+static inline bool fused_path(const gsr_system* s) { return s->tune.fused != 0; }
 
 extern "C" const char* gsr_strerror(int code) {
   switch (code) {
@@ -107,16 +108,19 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M) {
+static int make_row_tensor_map(CUtensorMap* map, const double* values, int64_t M, int cpr) {
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
     return cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
-  // pair view (tma.cuh): one tensor row = two matrix rows = 384 bytes; the last row of an odd M is not covered
-  const cuuint64_t dims[2] = {(cuuint64_t)(2 * NSLOT), (cuuint64_t)(M >= 2 ? M / 2 : 1)};
-  const cuuint64_t strides[1] = {(cuuint64_t)(2 * NSLOT) * sizeof(double)};
-  const cuuint32_t box[2] = {50u, 16u};                                      // 48 + 2 zero-filled pad columns
+  // group view (tma.cuh): one tensor row = a GROUP of matrix rows (two 192-byte or four 184-byte records: a whole number
+  // of 16-byte units, which the pitch needs); the last M mod GROUP rows are not covered (TileRing::acquire copies them)
+  const int group = cpr == NSLOT ? Rec24::GROUP : Rec23::GROUP;
+  const cuuint64_t dims[2] = {(cuuint64_t)(group * cpr), (cuuint64_t)(M >= group ? M / group : 1)};
+  const cuuint64_t strides[1] = {(cuuint64_t)(group * cpr) * sizeof(double)};
+  const cuuint32_t box[2] = {(cuuint32_t)(cpr == NSLOT ? Rec24::BOX_COLS : Rec23::BOX_COLS),      // the group + zero-filled pad columns
+                             (cuuint32_t)(TILE_ROWS / group)};
   const cuuint32_t estr[2] = {1u, 1u};
   CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(values),
                                                    dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -297,8 +301,8 @@ extern "C" int gsr_create(gsr_system** out, const gsr_layout* L, const double* v
     if (h != 0) { delete s; return GSR_ELAYOUT; }
   }
   // side structures: the row-tile tensor map, the interleaved attitude buffers, instrumental replicas
-  if (v.M > 0 && v.cpr == NSLOT) {
-    int rc = make_row_tensor_map(&s->side.map, values, v.M);
+  if (v.M > 0) {
+    int rc = make_row_tensor_map(&s->side.map, values, v.M, v.cpr);
     if (rc) { delete s; return rc; }
   }
   int rc2 = build_att_buffers(s);
@@ -357,7 +361,7 @@ extern "C" int gsr_attach_constraints(gsr_system* s, int64_t n_rows, const doubl
   if (h != 0) return GSR_ELAYOUT;
   s->con_side = s->side;                 // shares the attitude buffers and the instrumental replicas (never freed twice:
                                          // gsr_destroy frees `side` only)
-  if (c.cpr == NSLOT && (rc = make_row_tensor_map(&s->con_side.map, values, n_rows))) return rc;
+  if ((rc = make_row_tensor_map(&s->con_side.map, values, n_rows, c.cpr))) return rc;
   s->con = c;
   s->has_con = true;
   return GSR_OK;

@@ -15,7 +15,7 @@ namespace gsr {
 // v and g are LSQR-internal n-vectors: their attitude blocks are in the interleaved layout (aprod_device.cuh).
 // PART: with the L2 instrumental accumulators, the leading acc_part columns are accumulated in shared memory instead
 // (a template parameter: the kernel without them carries none of that code).
-template <bool GSMEM, bool ASMEM, bool PART>
+template <class REC, bool GSMEM, bool ASMEM, bool PART>
 __global__ void __launch_bounds__(MAX_TMA_WARPS * 32, 1)
 k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, const double* __restrict__ v,
              double* __restrict__ uh, double* __restrict__ g, InstrAcc ia, int use_tab, int tab_shift, int acc_part,
@@ -37,7 +37,7 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
   double* xi_s = acc_s + (ASMEM ? ((s.I + 1) & ~1ll) : ((acc_part + 1) & ~1));
   uint32_t* tab_s = reinterpret_cast<uint32_t*>(xi_s + (GSMEM ? ((s.I + 1) & ~1ll) : 0));
 
-  TileRing ring;
+  TileRing<REC> ring;
   const int64_t gw = (int64_t)blockIdx.x * nwarps + warp, W = (int64_t)gridDim.x * nwarps;
   ring.init(ring_mem, bars + warp * nstages, &map, s.vals, s.idx, s.M, gw, W, lane, nstages);
   const int64_t n_acc = ASMEM ? s.I : (PART ? acc_part : 0);   // accumulators privatised in shared memory: all, or the leading columns
@@ -67,24 +67,24 @@ k_lsqr_fused(const __grid_constant__ CUtensorMap map, SysView s, int nstages, co
     const int nvalid = (s.M - row0) < TILE_ROWS ? (int)(s.M - row0) : TILE_ROWS;
     char* tile = ring.acquire(t, lane);
     RowRegs row;
-    load_row(tile, lane, valid, row);
+    load_row<REC>(tile, lane, valid, row);
     int ts[16];
     att_starts(tile, al, ts);
     __syncwarp();   // every lane holds its row: the exchange runs may be written
-    att_gather(tile, al, ts, att_il);
+    att_gather<REC>(tile, al, ts, att_il);
     const double rest = row_dot_rest<GSMEM>(row, gc);
     __syncwarp();
-    double out = fma(c0, uin, att_dot_row(tile, lane, row) + rest);
+    double out = fma(c0, uin, att_dot_row<REC>(tile, lane, row) + rest);
     if (valid) {
       uh[r] = out;
       sq = fma(out, out, sq);
     } else {
       out = 0.0;
     }
-    att_products(tile, lane, row, out);
+    att_products<REC>(tile, lane, row, out);
     __syncwarp();
-    att_scatter(tile, al, ts, sc.gatt_il);
-    astro_scatter(tile, lane, nvalid, valid, row, out, sc.x);
+    att_scatter<REC>(tile, al, ts, sc.gatt_il);
+    astro_scatter<REC>(tile, lane, nvalid, valid, row, out, sc.x);
     gacc += scatter_rest<ASMEM, PART>(row, lane, valid, out, sc);
     ring.release(lane);
   }
@@ -116,8 +116,13 @@ cudaError_t launch_lsqr_fused(const SysView& s, const SideData& sd, const Tuning
   const bool use_copies = !p.acc_smem && p.ins_tab && sd.ins.chunk_tab != nullptr && t.instr_copies != 0;
   void (*k)(const CUtensorMap, SysView, int, const double*, double*, double*, InstrAcc, int, int, int, const double*, double*, int*);
   const bool part = use_copies && p.acc_part > 0;
-  if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<true, true, false> : (part ? k_lsqr_fused<true, false, true> : k_lsqr_fused<true, false, false>);
-  else k = p.acc_smem ? k_lsqr_fused<false, true, false> : (part ? k_lsqr_fused<false, false, true> : k_lsqr_fused<false, false, false>);
+  if (s.cpr == NSLOT) {
+    if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<Rec24, true, true, false> : (part ? k_lsqr_fused<Rec24, true, false, true> : k_lsqr_fused<Rec24, true, false, false>);
+    else k = p.acc_smem ? k_lsqr_fused<Rec24, false, true, false> : (part ? k_lsqr_fused<Rec24, false, false, true> : k_lsqr_fused<Rec24, false, false, false>);
+  } else {
+    if (p.gather_smem) k = p.acc_smem ? k_lsqr_fused<Rec23, true, true, false> : (part ? k_lsqr_fused<Rec23, true, false, true> : k_lsqr_fused<Rec23, true, false, false>);
+    else k = p.acc_smem ? k_lsqr_fused<Rec23, false, true, false> : (part ? k_lsqr_fused<Rec23, false, false, true> : k_lsqr_fused<Rec23, false, false, false>);
+  }
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
   if (e != cudaSuccess) return e;
   ++*launches;

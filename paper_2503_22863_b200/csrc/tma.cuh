@@ -19,14 +19,40 @@
 namespace gsr {
 
 constexpr int TILE_ROWS = 32;
-constexpr int PAIR_BYTES = 400;                                // two 192-byte rows + 16 bytes of zero pad
-constexpr int COEF_TILE_BYTES = (TILE_ROWS / 2) * PAIR_BYTES;  // 6400
+constexpr int COEF_TILE_BYTES = 6400;                          // staged coefficients of a tile, either record format
 constexpr int IDX_TILE_BYTES = TILE_ROWS * 32;                 // 1024
 constexpr int STAGE_BYTES = COEF_TILE_BYTES + IDX_TILE_BYTES;  // 7424 (multiple of 128)
 
-// byte offset of row r (0..31) of a staged tile, and of the 8-byte pad slot that belongs to it
-__host__ __device__ constexpr int row_off(int r) { return (r >> 1) * PAIR_BYTES + (r & 1) * 192; }
-__host__ __device__ constexpr int pad_off(int r) { return (r >> 1) * PAIR_BYTES + 384 + (r & 1) * 8; }
+// How the records of a tile lie in shared memory, per record format.  A GROUP of consecutive rows is one row of the
+// tensor view (a whole number of 16-byte units in HBM, which cuTensorMapEncodeTiled needs for its pitch); the box is a
+// few columns wider than the group, the out-of-bounds columns are zero-filled, and that pad (i) sets the group stride in
+// shared memory so that the lane-per-row loads are bank-conflict free and (ii) holds the group's y values (y_off).
+//   Rec24: 24 doubles per row (192 B).  Group = 2 rows = 384 B = three whole 128-byte lines; box 50 x 16; group stride
+//          400 B, rows 192 B apart: every row is 16-byte aligned, LDS.128 per lane, the chunk positions
+//          (25 * (l >> 1) + 12 * (l & 1) + c) mod 8 take each value exactly four times over a warp.
+//   Rec23: 23 doubles per row (184 B, the production record without the global slot).  184 B is 8-byte
+//          aligned only and 2 rows (368 B) are no whole number of 16-byte units, but 4 rows are: group = 4 rows = 736 B,
+//          view 92 x floor(M/4), box 100 x 8; group stride 800 B, rows 184 B apart.  Odd rows of a group are 8-byte
+//          aligned only, so the lanes use LDS.64: in 8-byte units lane l reads (100 * (l >> 2) + 23 * (l & 3) + c), and
+//          {4 g + 7 i mod 16 : g, i < 4} are 16 different values, i.e. each half-warp (one 128-byte wavefront of 8-byte
+//          accesses) touches 16 different bank pairs: conflict free.
+struct Rec24 {
+  static constexpr int CPR = 24, GROUP = 2, GROUP_SHIFT = 1, GROUP_BYTES = 400, BOX_COLS = 50, VIEW_COLS = 48;
+  static constexpr bool VEC16 = true;
+  __host__ __device__ static constexpr int row_off(int r) { return (r >> 1) * GROUP_BYTES + (r & 1) * 192; }
+  __host__ __device__ static constexpr int y_off(int r) { return (r >> 1) * GROUP_BYTES + 384 + (r & 1) * 8; }
+  // row 2 * it + h (h = 0, 1), the row a half-warp serves in pass `it` of the cooperative attitude routines
+  __host__ __device__ static constexpr int coop_off(int it, int h) { return it * GROUP_BYTES + h * 192; }
+};
+struct Rec23 {
+  static constexpr int CPR = 23, GROUP = 4, GROUP_SHIFT = 2, GROUP_BYTES = 800, BOX_COLS = 100, VIEW_COLS = 92;
+  static constexpr bool VEC16 = false;
+  __host__ __device__ static constexpr int row_off(int r) { return (r >> 2) * GROUP_BYTES + (r & 3) * 184; }
+  __host__ __device__ static constexpr int y_off(int r) { return (r >> 2) * GROUP_BYTES + 736 + (r & 3) * 8; }
+  __host__ __device__ static constexpr int coop_off(int it, int h) { return (it >> 1) * GROUP_BYTES + ((it & 1) * 2 + h) * 184; }
+};
+static_assert((TILE_ROWS / Rec24::GROUP) * Rec24::GROUP_BYTES == COEF_TILE_BYTES, "Rec24 tile");
+static_assert((TILE_ROWS / Rec23::GROUP) * Rec23::GROUP_BYTES == COEF_TILE_BYTES, "Rec23 tile");
 
 #ifdef GSR_HOST_EMULATION
 // tests/emu: the same helpers for the host build of the kernels (test infrastructure; never part of libgsr.so).
@@ -93,6 +119,7 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
 #endif  // GSR_HOST_EMULATION
 
 // Per-warp ring of `nstages` row tiles.  All 32 lanes call every method; lane 0 talks to the TMA.
+template <class REC>
 struct TileRing {
   char* base;       // this warp's STAGES * STAGE_BYTES of shared memory (128-byte aligned)
   uint64_t* bars;   // this warp's STAGES mbarriers
@@ -111,9 +138,9 @@ struct TileRing {
     const int64_t left = M - row0;
     const uint32_t idx_bytes = static_cast<uint32_t>((left < TILE_ROWS ? left : TILE_ROWS) * 32);
     char* dst = base + s * STAGE_BYTES;
-    const bool pairs = row0 + 1 < M;   // the tile holds at least one whole pair (else: a single last row)
+    const bool pairs = row0 + (REC::GROUP - 1) < M;   // the tile holds at least one whole group (else: only rows the warp copies)
     mbar_expect_tx(bars + s, (pairs ? COEF_TILE_BYTES : 0) + idx_bytes);
-    if (pairs) tma_load_2d(dst, map, 0, static_cast<int>(row0 >> 1), bars + s, policy);
+    if (pairs) tma_load_2d(dst, map, 0, static_cast<int>(row0 >> REC::GROUP_SHIFT), bars + s, policy);
     bulk_load_1d(dst + COEF_TILE_BYTES, idx + row0 * 8, idx_bytes, bars + s, policy);
   }
 
@@ -148,14 +175,28 @@ struct TileRing {
   __device__ __forceinline__ char* acquire(int64_t t, int lane) {
     mbar_wait(bars + stage, phase);
     char* tile = base + stage * STAGE_BYTES;
-    if ((M & 1) && t == n_tiles - 1) {
-      // odd M: the last row has no partner, so the pair view does not cover it.  The warp copies it
-      // (and clears the coefficient area first when the tile is that single row and no TMA load ran).
-      const int last = static_cast<int>(M - 1 - t * TILE_ROWS);
-      if (last == 0)
+    if (REC::GROUP == 2) {
+      if ((M & 1) && t == n_tiles - 1) {
+        // odd M: the last row has no partner, so the pair view does not cover it.  The warp copies it
+        // (and clears the coefficient area first when the tile is that single row and no TMA load ran).
+        const int last = static_cast<int>(M - 1 - t * TILE_ROWS);
+        if (last == 0)
+          for (int i = lane; i < COEF_TILE_BYTES / 16; i += 32) reinterpret_cast<int4*>(tile)[i] = make_int4(0, 0, 0, 0);
+        __syncwarp();
+        if (lane < 24) reinterpret_cast<double*>(tile + REC::row_off(last))[lane] = vals[(M - 1) * 24 + lane];
+        __syncwarp();
+      }
+    } else if ((M & (REC::GROUP - 1)) && t == n_tiles - 1) {
+      // the last M mod GROUP rows have no whole group, so the tensor view does not cover them.  The warp copies
+      // them (and clears the coefficient area first when the tile holds nothing else and no TMA load ran).
+      const int64_t tail0 = M & ~static_cast<int64_t>(REC::GROUP - 1);   // first row of the tail; it lies in this, the last, tile
+      const int first = static_cast<int>(tail0 - t * TILE_ROWS);
+      if (first == 0)
         for (int i = lane; i < COEF_TILE_BYTES / 16; i += 32) reinterpret_cast<int4*>(tile)[i] = make_int4(0, 0, 0, 0);
       __syncwarp();
-      if (lane < 24) reinterpret_cast<double*>(tile + row_off(last))[lane] = vals[(M - 1) * 24 + lane];
+      for (int64_t r = tail0; r < M; r++)
+        if (lane < REC::CPR)
+          reinterpret_cast<double*>(tile + REC::row_off(first + static_cast<int>(r - tail0)))[lane] = vals[r * REC::CPR + lane];
       __syncwarp();
     }
     return tile;

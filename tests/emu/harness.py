@@ -87,6 +87,9 @@ def fake_cuda_queries():
 def emulated(*modules):
     """Inside the block paper_2503_22863_b200.binding talks to the emulated library; `modules` (GPU test modules) get
     DEV = "cpu" and a dev() that makes aligned host copies.  Everything is put back afterwards."""
+    # helpers are shared between the GPU test modules (test_gpu_zzzz_coeff23 calls into test_gpu_z_f3): patch them all
+    modules = list(modules) + [m for name, m in list(sys.modules.items())
+                               if (name.startswith("test_gpu_") or name == "gpu_helpers") and m not in modules]
     saved = (binding._lib, binding._dev_ptr, binding._stream, binding.GsrSystem.exchange_buffer)
     saved_mod = [(m, getattr(m, "DEV", None), getattr(m, "dev", None), getattr(m, "gdev", None)) for m in modules]
     binding._lib = emu_lib()

@@ -62,16 +62,24 @@ CASES = [
     ("test_gpu_precond", "test_colnorms", ("C1",), False),
     ("test_gpu_precond", "test_colnorms", ("C5-small",), True),
     ("test_gpu_precond", "test_preconditioned_solve", ("*",), False),
-    ("test_gpu_z_f3", "test_coeff23_products", (1, 1), True),
-    ("test_gpu_z_f3", "test_coeff23_products", (1, 33), True),
-    ("test_gpu_z_f3", "test_coeff23_products", (3, 11), False),
-    ("test_gpu_z_f3", "test_coeff23_products", (7, 37), True),
-    ("test_gpu_z_f3", "test_coeff23_products", (64, 64), False),
-    ("test_gpu_z_f3", "test_coeff23_products", (40, 100), False),
-    ("test_gpu_z_f3", "test_coeff23_lsqr", (), False),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 1), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 2), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 3), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 33), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 34), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (1, 35), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (3, 10), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (3, 11), False),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (7, 37), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (5, 129), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (64, 64), False),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (40, 100), False),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (300, 1), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_products", (41, 5), True),
+    ("test_gpu_zzzz_coeff23", "test_coeff23_lsqr", (), False),
     ("test_gpu_z_f3", "test_constraint_section_24", (1,), False),
     ("test_gpu_z_f3", "test_constraint_section_24", (0,), False),
-    ("test_gpu_z_f3", "test_constraint_section_coeff23", (), False),
+    ("test_gpu_zzzz_coeff23", "test_constraint_section_coeff23", (), True),
     ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (1, 300), False),
     ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (2, 300), False),
     ("test_gpu_zz_sharded", "test_sharded_lsqr_against_oracle", (3, 300), False),
@@ -83,6 +91,7 @@ CASES = [
     ("test_gpu_zzz_deterministic", "test_deterministic_aprod2", (300, 1), False),
     ("test_gpu_zzz_deterministic", "test_deterministic_aprod2_skewed_stars_and_sections", (), True),
     ("test_gpu_zzz_deterministic", "test_lsqr_two_pass_with_deterministic_aprod2", (), True),
+    ("test_gpu_zzzz_coeff23", "test_deterministic_aprod2_coeff23_with_constraint_section", (), True),
 ]
 
 

@@ -1,6 +1,5 @@
-"""GPU parity for SURVEY.md section 8(f3): the 23-coefficient production record (GSR_LAYOUT_COEFF23, N_Glob = 0,
-PAPER.md:141) and the constraint equations as a section of their own (gsr_attach_constraints),
-against the CPU oracle on the same seeded inputs.  The oracle sees ONE matrix [A_obs; A_con] (that is the
+"""GPU parity for SURVEY.md section 8(f3): the constraint equations as a section of their own (gsr_attach_constraints,
+PAPER.md:41, 72), against the CPU oracle on the same seeded inputs (the 23-coefficient record: test_gpu_zzzz_coeff23.py).  The oracle sees ONE matrix [A_obs; A_con] (that is the
 definition of "a section appended after the observation rows") in the storage under test.
 
 Tolerances as everywhere (readings R14, R15, R16): aprod 1 per row 1e-13 of the forward bound, aprod 2
@@ -87,48 +86,6 @@ def check_lsqr(shape, L, a, idx, s, early=(1, 2, 3, 5), with_replay=True):
         replay_one_step(shape, a, idx, s)
 
 
-# ------------------------------------------------------------------ the 23-coefficient record
-@pytest.mark.parametrize("n_stars,obs", [(1, 1), (1, 33), (3, 11), (7, 37), (64, 64), (40, 100)])
-def test_coeff23_products(n_stars, obs):
-    shape = tiny_shape(n_stars=n_stars, obs=obs, n_knots=12, n_instr=9, n_glob=0, seed=230 + n_stars)
-    a24, idx = host.make_rows(shape)
-    a23 = np.ascontiguousarray(a24[:, :23])
-    L23 = oracle.layout(shape.n_stars, shape.n_knots, shape.n_instr, 0, coeffs_per_row=23)
-    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, dev(a23), dev(idx), coeffs_per_row=23) as s:
-        check_products(shape, L23, a23, idx, s, seed=31)
-        check_colnorms(L23, a23, idx, s)
-    # duplicates inside a row, and the record refused with a global parameter
-    idx2 = idx.copy()
-    idx2[::3, 2:8] = np.array([1, 1, 3, 0, 5, 3], dtype=np.int32)
-    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, dev(a23), dev(idx2), coeffs_per_row=23) as s:
-        check_products(shape, L23, a23, idx2, s, seed=32)
-        check_colnorms(L23, a23, idx2, s)
-    with pytest.raises(gsr.GsrError) as ei:
-        gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 1, dev(a23), dev(idx), coeffs_per_row=23)
-    assert ei.value.code == -1
-
-
-def test_coeff23_lsqr():
-    shape = tiny_shape(n_stars=60, obs=25, n_knots=40, n_instr=12, n_glob=0, seed=2325)
-    a24, idx = host.make_rows(shape)
-    a23 = np.ascontiguousarray(a24[:, :23])
-    L23 = oracle.layout(shape.n_stars, shape.n_knots, shape.n_instr, 0, coeffs_per_row=23)
-    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, dev(a23), dev(idx), coeffs_per_row=23) as s:
-        check_lsqr(shape, L23, a23, idx, s)
-        # the same solve in the 24-slot storage of the same system gives the same solution
-        x23 = torch.empty(shape.n_unknowns, dtype=torch.float64, device=DEV)
-        b = dev(rhs(shape, a24, idx, host.x_true(shape)))
-        s.lsqr(b, x23, 5000, 1e-12, 1e-12, 1e8)
-        with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, dev(a24), dev(idx)) as s24:
-            x24 = torch.empty_like(x23)
-            s24.lsqr(b, x24, 5000, 1e-12, 1e-12, 1e8)
-        assert float(torch.linalg.norm(x23 - x24)) <= 1e-9 * float(torch.linalg.norm(x24))
-        # the preconditioned operator exists on the fused (24-slot) path only
-        with pytest.raises(gsr.GsrError) as ei:
-            s.lsqr_ex(b, x23, precond=True, itnlim=3)
-        assert ei.value.code == -5
-
-
 # ------------------------------------------------------------------ the constraint section
 def constraint_system(n_glob):
     shape = C5.scaled(150, n_knots=200, n_instr=300, n_constraint_rows=46, n_glob=n_glob, name="C5-small")
@@ -166,16 +123,3 @@ def test_constraint_section_24(n_glob):
         s.attach_constraints(None, None)
         assert s.n_rows == m_obs
         check_products(shape, L, a[:m_obs], idx[:m_obs], s, seed=42)
-
-
-def test_constraint_section_coeff23():
-    shape, a, idx, m_obs = constraint_system(0)
-    a23 = np.ascontiguousarray(a[:, :23])
-    L23 = oracle.layout(shape.n_stars, shape.n_knots, shape.n_instr, 0, coeffs_per_row=23)
-    av, iv = dev(a23), dev(idx)
-    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, av[:m_obs], iv[:m_obs], coeffs_per_row=23) as s:
-        s.attach_constraints(av[m_obs:], iv[m_obs:])
-        assert s.n_rows == a.shape[0]
-        check_products(shape, L23, a23, idx, s, seed=43)
-        check_colnorms(L23, a23, idx, s)
-        check_lsqr(shape, L23, a23, idx, s, early=(1, 3))

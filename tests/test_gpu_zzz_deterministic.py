@@ -5,7 +5,8 @@ csrc/aprod2_det.cu): every sum has one fixed order that depends on the sizes onl
   rounding only);
 * with det_chunks = 1 the order is the CPU oracle's own (row by row, slot by slot, from x's initial value, no FMA
   contraction), so the result is bit-identical to oracle.aprod2 -- both record formats, repeated instrumental columns,
-  a constraint section attached (the oracle then sees the one matrix [A_obs; A_con]);
+  a constraint section attached (the oracle then sees the one matrix [A_obs; A_con]); the 23-coefficient record:
+  test_gpu_zzzz_coeff23.py;
 * with any chunk count it meets the usual aprod 2 tolerance (reading R15);
 * LSQR on the two-pass schedule with this aprod 2 follows the default solve (k = 5, reading R16).
 (File name sorts last among the GPU tests.)"""
@@ -67,16 +68,14 @@ def test_deterministic_aprod2_skewed_stars_and_sections():
     a, idx = host.make_rows(shape)
     with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, dev(a), dev(idx)) as s:
         check_variant2(shape, oracle.layout_of(shape), a, idx, s, seed=52)
-    # 23-coefficient record, with the constraint rows as a section of their own
-    shape = C5.scaled(40, n_knots=60, n_instr=30, n_constraint_rows=14, n_glob=0, name="C5-tiny")
-    a24, idx = host.make_rows(shape)
-    a23 = np.ascontiguousarray(a24[:, :23])
+    # with the constraint rows as a section of their own (the oracle sees the one matrix [A_obs; A_con])
+    shape = C5.scaled(40, n_knots=60, n_instr=30, n_constraint_rows=14, name="C5-tiny")
+    a, idx = host.make_rows(shape)
     m_obs = shape.n_stars * shape.obs_per_star
-    L23 = oracle.layout(shape.n_stars, shape.n_knots, shape.n_instr, 0, coeffs_per_row=23)
-    av, iv = dev(a23), dev(idx)
-    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, 0, av[:m_obs], iv[:m_obs], coeffs_per_row=23) as s:
+    av, iv = dev(a), dev(idx)
+    with gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, av[:m_obs], iv[:m_obs]) as s:
         s.attach_constraints(av[m_obs:], iv[m_obs:])
-        check_variant2(shape, L23, a23, idx, s, seed=53)
+        check_variant2(shape, oracle.layout_of(shape), a, idx, s, seed=53)
 
 
 def test_lsqr_two_pass_with_deterministic_aprod2():
