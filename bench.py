@@ -54,6 +54,8 @@ def parse():
     ap.add_argument("--coeff23", action="store_true",
                     help="control: the same workload with N_Glob = 0 in the 23-coefficient production record (184-byte rows, "
                          "GSR_LAYOUT_COEFF23) instead of the padded 24-slot record")
+    ap.add_argument("--n-glob", type=int, default=-1, choices=[-1, 0, 1],
+                    help="control: override the workload's N_Glob (0 = the padded 24-slot record of the system --coeff23 stores in 23)")
     ap.add_argument("--reps", type=int, default=20, help="repetitions of the single aprod 1 / aprod 2 timings")
     ap.add_argument("--cov-pairs", type=int, action="append", default=[], help="--mode extras: pair counts to time")
     return ap.parse_args()
@@ -313,6 +315,9 @@ def run_gsr(args):
         return run_extras(args, shape, dev, rank, world)
 
     cpr = 24
+    if args.n_glob >= 0 and not args.coeff23:
+        from dataclasses import replace
+        shape = replace(shape, n_glob=args.n_glob, name=shape.name + f"[N_Glob = {args.n_glob}]")
     if args.coeff23:
         # the production record: N_Glob = 0, 23 doubles per row.  Generated block by block (the 24-slot rows of a block,
         # slots 0..22 packed) so that C4 never holds both storages.
