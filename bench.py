@@ -54,6 +54,9 @@ def parse():
     ap.add_argument("--coeff23", action="store_true",
                     help="control: the same workload with N_Glob = 0 in the 23-coefficient production record (184-byte rows, "
                          "GSR_LAYOUT_COEFF23) instead of the padded 24-slot record")
+    ap.add_argument("--sharded", action="store_true",
+                    help="SURVEY.md 8(f2): ONE system row-sharded over the ranks (strong scaling) instead of one replica per "
+                         "rank; the default for --gpus N stays replicas (BASELINE.json north_star: one GPU)")
     ap.add_argument("--n-glob", type=int, default=-1, choices=[-1, 0, 1],
                     help="control: override the workload's N_Glob (0 = the padded 24-slot record of the system --coeff23 stores in 23)")
     ap.add_argument("--reps", type=int, default=20, help="repetitions of the single aprod 1 / aprod 2 timings")
@@ -313,6 +316,8 @@ def run_gsr(args):
     K, W = args.steps, max(args.warmup, 3)
     if args.mode == "extras":
         return run_extras(args, shape, dev, rank, world)
+    if args.sharded:
+        return run_sharded(args, shape, dev, rank, world, K, W)
 
     cpr = 24
     if args.n_glob >= 0 and not args.coeff23:
@@ -480,6 +485,80 @@ def run_gsr(args):
         except Exception as ex:                                    # noqa: BLE001
             line["e2e"] = {"value": None, "unit": "ms", "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
                            "note": f"failed: {type(ex).__name__}: {ex}"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_sharded(args, shape, dev, rank, world, K, W):
+    """--sharded: the workload's rows cut at star boundaries into one range per rank (paper_2503_22863_b200/sharded.py),
+    every rank generating only its own rows; the constraint rows, if any, are rank 0's second section.  K iterations of
+    the sharded solve are timed (phases + one NCCL allreduce per exchange), max over ranks.  Strong scaling: the job is
+    the same system whatever N."""
+    import torch
+    import torch.distributed as dist
+    import paper_2503_22863_b200 as gsr
+    from gaia_synth import configs as C
+    from gaia_synth import device as gdev
+    from gaia_synth import host
+    from paper_2503_22863_b200.sharded import DistComm, LocalComm, ShardedLsqr, partition_stars
+    counts = (shape.n_stars, shape.obs_per_star) if shape.obs_per_star else host.obs_counts(shape)
+    part = partition_stars(counts, world)[rank]
+    m_obs = host.n_obs_rows(shape)
+    vals, idx = gdev.make_system(shape, device=dev, r0=part.row_lo, r1=part.row_hi)
+    sysm = gsr.gsr_create(shape.n_stars, shape.n_knots, shape.n_instr, shape.n_glob, vals, idx)
+    for opt in args.option:
+        k, v = opt.split("=")
+        sysm.set_option(k, int(v))
+    noise = [gdev.normal(shape.seed, C.STREAM_NOISE, part.row_lo, part.row_hi, scale=shape.sigma, device=dev)]
+    con = None
+    if rank == 0 and shape.n_constraint_rows:
+        con = gdev.make_system(shape, device=dev, r0=m_obs, r1=m_obs + shape.n_constraint_rows)
+        sysm.attach_constraints(*con)
+        noise.append(gdev.normal(shape.seed, C.STREAM_NOISE, m_obs, m_obs + shape.n_constraint_rows, scale=shape.sigma, device=dev))
+    b = torch.cat(noise)
+    sysm.aprod1(gdev.x_true(shape, device=dev), b)          # this rank's rows of b = A x_true + noise
+    m_local, n = sysm.n_rows, shape.n_unknowns
+    m_total = host.n_rows(shape)
+    drv = ShardedLsqr([sysm], DistComm() if world > 1 else LocalComm(1), check_every=1 << 30)
+    stopped, _ = drv.begin([b], 1 << 40)
+    assert not stopped
+    drv.iterate(W)
+    torch.cuda.synchronize()
+    l0 = sysm.launch_count()
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    drv.iterate(K)
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_iter = max_over_ranks(e0.elapsed_time(e1), dev) / K
+    stopped, res = drv.poll()
+    assert res.itn == W + K and not stopped
+    ab = algorithmic_bytes(m_total, n)
+    peak, _ = measured_peak()
+    ns = n - 5 * shape.n_stars
+    line = {"metric": "ms_per_lsqr_iteration", "value": ms_iter, "unit": "ms", "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_iter, "higher_is_better": False, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"{shape.name}: {m_total} rows x {n} unknowns, row-sharded over {world} rank(s) at star "
+                                   f"boundaries (rank 0: {m_local} rows)",
+                       "parallelism": f"row-sharded x{world} (gsr_shard_* phases; one allreduce of {ns + 2} doubles and one of 1 "
+                                      "double per iteration)",
+                       "l2_policy": "inputs (matrix) far larger than L2; no flush", "options": args.option},
+            "iteration_effective_gbs_two_pass_formula": ab["iteration"] / (ms_iter * 1e-3) / 1e9,
+            "iteration_effective_frac_of_8TBs_per_gpu": ab["iteration"] / (ms_iter * 1e-3) / 1e9 / NOMINAL_HBM_GBS / world,
+            "gpu_launches": sysm.launch_count() - l0, "exchanges_per_iteration": 2,
+            "exchanged_bytes_per_iteration_per_rank": 8 * (ns + 3), "clocks": clocks,
+            "lsqr": {"itn": res.itn, "istop": res.istop, "r1norm": res.r1norm, "anorm": res.anorm}}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

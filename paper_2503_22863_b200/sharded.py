@@ -140,24 +140,40 @@ class ShardedLsqr:
             raise RuntimeError("shards disagree on the stop flag")
         return stopped, polls[0][1]
 
-    def solve(self, bs, itnlim, atol=0.0, btol=0.0, conlim=0.0):
-        """bs: this process's right-hand sides, one per local shard (each the shard's own rows of b).
-        Returns the LsqrResult every rank agrees on."""
+    def begin(self, bs, itnlim, atol=0.0, btol=0.0, conlim=0.0):
+        """Start a solve: bs = this process's right-hand sides, one per local shard (each the shard's own rows of b).
+        Runs the initialisation phases with their exchanges; returns (stopped, LsqrResult) of the first poll
+        (stopped already when b = 0 or A^T b = 0: x = 0 is the solution)."""
         bs = list(bs)
         if len(bs) != len(self.shards):
             raise ValueError("one right-hand side per local shard")
         self.exchanges = self.exchanged_doubles = self.iterations = 0
+        self.itnlim = int(itnlim)
         counts = [sh.shard_begin(b, xb, self.comm.counts_shared(i), itnlim, atol, btol, conlim)
                   for i, (sh, b, xb) in enumerate(zip(self.shards, bs, self.xbufs))]
         self._exchange(counts)
         while self._phase() != SHARD_INIT_DONE:
             pass
-        stopped, res = self._poll()                    # (b = 0 or A^T b = 0: x = 0 is the solution)
+        return self._poll()
+
+    def iterate(self, n_iters: int):
+        """n_iters more LSQR iterations on every rank, in lock step, without looking at the stop flag (iterations after a
+        stop are no-ops on the device, as in gsr_lsqr_iterate).  Asynchronous apart from the exchanges."""
+        for _ in range(int(n_iters)):
+            while self._phase() != SHARD_ITER_DONE:
+                pass
+            self.iterations += 1
+
+    def poll(self):
+        """(stopped, LsqrResult): the device-side stop flag and scalars, identical on every rank.  Synchronises."""
+        return self._poll()
+
+    def solve(self, bs, itnlim, atol=0.0, btol=0.0, conlim=0.0):
+        """The whole solve; returns the LsqrResult every rank agrees on.  The stop flag is polled every check_every iterations."""
+        stopped, res = self.begin(bs, itnlim, atol, btol, conlim)
         while not stopped and self.iterations < itnlim:
-            if self._phase() == SHARD_ITER_DONE:
-                self.iterations += 1
-                if self.iterations % self.check_every == 0 or self.iterations >= itnlim:
-                    stopped, res = self._poll()
+            self.iterate(min(self.check_every - self.iterations % self.check_every, itnlim - self.iterations))
+            stopped, res = self._poll()
         if not stopped:                                # itnlim = 0
             stopped, res = self._poll()
         return res

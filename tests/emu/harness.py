@@ -55,6 +55,11 @@ class HostGen:
         return host_tensor(a), host_tensor(idx)
 
     @staticmethod
+    def normal(seed, stream_id, i0, i1, scale=1.0, device="cpu"):
+        from gaia_synth import host
+        return host_tensor(host.normal(seed, stream_id, i0, i1) * scale)
+
+    @staticmethod
     def x_true(shape, device="cpu"):
         from gaia_synth import host
         return host_tensor(host.x_true(shape))
