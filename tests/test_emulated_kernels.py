@@ -9,7 +9,7 @@ checked by the tests that did pass on hardware in round 1 (they pass here too). 
 about the hardware (timing, the async proxy, the real TMA / tensor-core units); the GPU tests remain the parity
 tests proper.  The emulated library is test infrastructure: the product never loads it and has no CPU fallback.
 
-Default: a subset that runs in about two minutes on 8 cores.  GSR_EMU_FULL=1 runs every GPU test body that fits the host
+Default: a subset that runs in about a minute on 8 cores.  GSR_EMU_FULL=1 runs every GPU test body that fits the host
 (all but the full-size C2...C5 systems, which are dry-run on small stand-in shapes).
 """
 import importlib
@@ -123,6 +123,7 @@ def test_gpu_test_body_on_host_emulation(modname, fn, args, fast):
 
 
 # ---- the full-size test bodies, dry-run on small stand-in shapes (their logic, not their size)
+@pytest.mark.skipif(not FULL, reason="GSR_EMU_FULL=1 runs it")
 def test_xl_oracle_test_bodies_on_small_shapes():
     X = importlib.import_module("test_gpu_xl_oracle")
     gpu_helpers = importlib.import_module("gpu_helpers")
@@ -139,6 +140,7 @@ def test_xl_oracle_test_bodies_on_small_shapes():
         X.SLICE_CASE, X.REPLAY_SHAPE, X.c5_shape = saved
 
 
+@pytest.mark.skipif(not FULL, reason="GSR_EMU_FULL=1 runs it")
 def test_partial_shared_memory_accumulators_and_private_table():
     """Options that are off by default because they were never timed in their committed form (acc_part, acc_part_fused:
     the PART = true kernel instances; tab_private): parity against the oracle at I = 60,000, rows that hit both sides
