@@ -31,8 +31,13 @@ __device__ __forceinline__ double ld_nc_na(const double* p) { return __ldg(p); }
 
 #ifdef GSR_HOST_EMULATION
 // (tests/emu: host build of the kernels; an atomic add stands in for the L2 reduction)
-__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
-__device__ __forceinline__ void red_add_if_ge(double* p, double v, int a, int b) { if (a >= b) atomicAdd(p, v); }
+__device__ __forceinline__ void red_add(double* p, double v, const std::source_location loc = std::source_location::current()) {
+  atomicAdd(p, v, loc);
+}
+__device__ __forceinline__ void red_add_if_ge(double* p, double v, int a, int b,
+                                              const std::source_location loc = std::source_location::current()) {
+  if (a >= b) atomicAdd(p, v, loc);
+}
 #else
 // fp64 reduction at L2, fire and forget.  Explicitly .global: a pointer that was read from a table in
 // shared memory would otherwise compile to a GENERIC atomic (no RED, address-space check per lane).

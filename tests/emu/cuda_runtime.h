@@ -17,6 +17,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <functional>
+#include <source_location>
 
 // ---- qualifiers ---------------------------------------------------------------------------------------------
 #define __global__
@@ -48,6 +49,22 @@ void dmma884(double& c0, double& c1, double a, double b);   // mma.sync.m8n8k4.f
 unsigned smid();
 void tensor_load_2d(void* dst, const CUtensorMap* map, int c0, int c1);
 void bulk_copy(void* dst, const void* src, uint32_t bytes);
+// request counting (tests/emu/count_requests.py): every hooked global access is logged per thread and grouped per warp
+// instruction afterwards.  kind: 0 = read-only gather (__ldg), 1 = fp64 reduction / atomic, 2 = TMA / bulk copy
+extern bool g_counting;
+void count_access(int kind, const void* addr, unsigned bytes, unsigned site);
+// site = source line + (1 << 20) when the access is made by the per-tile device routines (aprod_device.cuh), i.e. inside
+// the row loop of a matrix kernel, as opposed to a kernel prologue / epilogue or an n-length kernel
+static inline unsigned site_of(const std::source_location& loc) {
+  const char* f = loc.file_name();
+  const char* e = f;
+  while (*e) e++;
+  const char tail[] = "aprod_device.cuh";
+  const int n = (int)sizeof(tail) - 1;
+  bool tile = (e - f) >= n;
+  for (int i = 0; tile && i < n; i++) tile = e[i - n] == tail[i];
+  return loc.line() + (tile ? (1u << 20) : 0u);
+}
 }  // namespace emu
 #define threadIdx emu::t_threadIdx
 #define blockIdx emu::t_blockIdx
@@ -71,13 +88,17 @@ template <class T> static inline T __shfl_sync(unsigned, T v, int src) {
 template <class T> static inline T __shfl_xor_sync(unsigned m, T v, int lane_mask) {
   return __shfl_sync(m, v, (int)((emu::t_threadIdx.x & 31u) ^ (unsigned)lane_mask));
 }
-template <class T> static inline T __ldg(const T* p) { return *p; }
+template <class T> static inline T __ldg(const T* p, const std::source_location loc = std::source_location::current()) {
+  if (emu::g_counting) emu::count_access(0, p, sizeof(T), emu::site_of(loc));
+  return *p;
+}
 template <class T> static inline T __ldcs(const T* p) { return *p; }
 static inline size_t __cvta_generic_to_shared(const void* p) { return reinterpret_cast<size_t>(p); }
 static inline long long clock64() {
   return (long long)std::chrono::steady_clock::now().time_since_epoch().count();
 }
-static inline double atomicAdd(double* p, double v) {
+static inline double atomicAdd(double* p, double v, const std::source_location loc = std::source_location::current()) {
+  if (emu::g_counting) emu::count_access(1, p, 8, emu::site_of(loc));
   std::atomic_ref<double> a(*p);
   double old = a.load(std::memory_order_relaxed);
   while (!a.compare_exchange_weak(old, old + v, std::memory_order_relaxed)) {}

@@ -5,10 +5,15 @@
 // barrier in a kernel is a real data race here too (ThreadSanitizer can see it).  "Device" memory is the heap.
 #include "cuda_runtime.h"
 
+#include <algorithm>
 #include <condition_variable>
 #include <cstdio>
+#include <map>
 #include <mutex>
+#include <set>
+#include <string>
 #include <thread>
+#include <tuple>
 #include <vector>
 
 #if defined(__SANITIZE_ADDRESS__)
@@ -67,6 +72,73 @@ static Barrier g_block_bar;
 static WarpState g_warps[MAX_THREADS / 32];
 thread_local WarpState* t_warp = nullptr;
 
+// ---- request counting ---------------------------------------------------------------------------------------------
+// Every hooked access of a thread is one record (kind, site = source line of the call, occurrence number of that site in
+// this thread, address).  The lanes of a warp run the same code, so (site, occurrence) names one warp instruction; at
+// the end of a block the records of each warp are grouped by it and the distinct 128-byte lines ("requests") and
+// 32-byte sectors of every instruction are added to the totals of the class its addresses fall into.
+bool g_counting = false;
+struct Rec { unsigned kind, site, epoch, occ; uintptr_t addr; unsigned bytes; };
+thread_local unsigned t_epoch = 0;      // warp rendezvous passed by this thread: the same for all lanes of a warp at any point of the code
+static std::vector<Rec> g_logs[MAX_THREADS];
+static std::map<unsigned long long, unsigned> g_occ[MAX_THREADS];
+struct Region { uintptr_t lo, hi; std::string name; };
+static std::vector<Region> g_regions;
+struct Tot { unsigned long long instr = 0, lanes = 0, lines = 0, sectors = 0; };
+static std::map<std::pair<int, std::string>, Tot> g_totals;       // (kind, class) -> totals
+static std::mutex g_count_mutex;
+
+void count_access(int kind, const void* addr, unsigned bytes, unsigned site) {
+  const uintptr_t a = reinterpret_cast<uintptr_t>(addr);
+  if (a >= reinterpret_cast<uintptr_t>(smem_raw) && a < reinterpret_cast<uintptr_t>(smem_raw) + SMEM_TOTAL) return;   // shared memory
+  const unsigned tid = t_threadIdx.x;
+  const unsigned long long key = ((unsigned long long)t_epoch << 32) | (site * 4u + (unsigned)kind);
+  g_logs[tid].push_back(Rec{(unsigned)kind, site, t_epoch, g_occ[tid][key]++, a, bytes});
+}
+// every emuMalloc block is a region too; blocks of exactly n doubles are n-vectors and are split by parameter block
+static unsigned long long g_n_bytes = 0, g_oA = 0, g_oI = 0, g_oG = 0, g_m_bytes = 0;
+static std::vector<Region> g_allocs;
+static std::string classify(uintptr_t a) {
+  for (const Region& r : g_regions)
+    if (a >= r.lo && a < r.hi) return r.name;
+  for (const Region& r : g_allocs)
+    if (a >= r.lo && a < r.hi) {
+      const unsigned long long sz = r.hi - r.lo, off = a - r.lo;
+      if (sz == g_n_bytes) return off < g_oA ? "n-vector: astrometric block" : off < g_oI ? "n-vector: attitude block"
+                                  : off < g_oG ? "n-vector: instrumental block" : "n-vector: global";
+      if (sz == g_m_bytes) return "M-vector";
+      return "library buffer of " + std::to_string(sz) + " B";
+    }
+  return "other";
+}
+void note_alloc(void* p, size_t bytes) {
+  std::lock_guard<std::mutex> lk(g_count_mutex);
+  g_allocs.push_back(Region{reinterpret_cast<uintptr_t>(p), reinterpret_cast<uintptr_t>(p) + bytes, ""});
+}
+void note_free(void* p) {
+  std::lock_guard<std::mutex> lk(g_count_mutex);
+  for (size_t i = 0; i < g_allocs.size(); i++)
+    if (g_allocs[i].lo == reinterpret_cast<uintptr_t>(p)) { g_allocs.erase(g_allocs.begin() + i); break; }
+}
+static void fold_block(unsigned block) {
+  std::lock_guard<std::mutex> lk(g_count_mutex);
+  for (unsigned w = 0; w * 32 < block; w++) {
+    std::map<std::tuple<unsigned, unsigned, unsigned, unsigned>, std::vector<const Rec*>> by_instr;
+    for (unsigned l = w * 32; l < std::min(block, w * 32 + 32); l++)
+      for (const Rec& r : g_logs[l]) by_instr[{r.kind, r.site, r.epoch, r.occ}].push_back(&r);
+    for (auto& [key, recs] : by_instr) {
+      std::set<uintptr_t> lines, sectors;
+      for (const Rec* r : recs) {
+        for (uintptr_t b = r->addr; b < r->addr + r->bytes; b += 8) { lines.insert(b >> 7); sectors.insert(b >> 5); }
+      }
+      const bool in_row_loop = std::get<0>(key) == 2 || (std::get<1>(key) >> 20) != 0;
+      Tot& t = g_totals[{(int)std::get<0>(key), (in_row_loop ? "" : "[outside the row loop] ") + classify(recs[0]->addr)}];
+      t.instr += 1; t.lanes += recs.size(); t.lines += lines.size(); t.sectors += sectors.size();
+    }
+  }
+  for (unsigned l = 0; l < block; l++) { g_logs[l].clear(); g_occ[l].clear(); }
+}
+
 // ---- thread pool ------------------------------------------------------------------------------------------------
 struct Pool {
   std::mutex m;
@@ -90,6 +162,7 @@ struct Pool {
       t_threadIdx = dim3{(unsigned)tid, 0, 0};
       t_blockIdx = bidx; t_blockDim = bdim; t_gridDim = gdim;
       t_warp = &g_warps[tid >> 5];
+      t_epoch = 0;
       (*body)();
       t_warp->bar.drop();
       g_block_bar.drop();
@@ -123,6 +196,7 @@ struct Pool {
     std::unique_lock<std::mutex> lk(m);
     cv_done.wait(lk, [&] { return n_done == n_active; });
     n_active = 0;      // late wake-ups of idle workers must not pick the finished job up
+    if (g_counting) fold_block(block);
   }
   ~Pool() {
     {
@@ -168,10 +242,11 @@ void launch(unsigned grid, unsigned block, size_t smem_bytes, void* stream, std:
 }
 
 void syncthreads() { g_block_bar.arrive_and_wait(); }
-void syncwarp() { t_warp->bar.arrive_and_wait(); }
+void syncwarp() { ++t_epoch; t_warp->bar.arrive_and_wait(); }
 
 uint64_t shfl(uint64_t v, int src_lane) {
   WarpState* w = t_warp;
+  ++t_epoch;
   w->xch[t_threadIdx.x & 31] = v;
   w->bar.arrive_and_wait();
   const uint64_t r = w->xch[src_lane];
@@ -184,6 +259,7 @@ uint64_t shfl(uint64_t v, int src_lane) {
 void dmma884(double& c0, double& c1, double a, double b) {
   WarpState* w = t_warp;
   const int lane = (int)(t_threadIdx.x & 31);
+  ++t_epoch;
   w->ma[lane] = a;
   w->mb[lane] = b;
   w->bar.arrive_and_wait();
@@ -206,13 +282,20 @@ void tensor_load_2d(void* dst, const CUtensorMap* map, int c0, int c1) {
   const long long pitch = (long long)map->opaque[3] / 8;
   const int b0 = (int)map->opaque[4], b1 = (int)map->opaque[5];
   double* out = static_cast<double*>(dst);
+  if (g_counting) {                                   // the in-bounds part of the box, one contiguous run of whole groups
+    const long long rows = std::max(0LL, std::min((long long)b1, d1 - c1));
+    if (rows > 0 && c0 == 0) count_access(2, base + (long long)c1 * pitch, (unsigned)(rows * pitch * 8), 2);
+  }
   for (int j = 0; j < b1; j++)
     for (int i = 0; i < b0; i++) {
       const long long c = c0 + i, r = (long long)c1 + j;
       out[(size_t)j * b0 + i] = (c >= 0 && c < d0 && r >= 0 && r < d1) ? base[r * pitch + c] : 0.0;
     }
 }
-void bulk_copy(void* dst, const void* src, uint32_t bytes) { std::memcpy(dst, src, bytes); }
+void bulk_copy(void* dst, const void* src, uint32_t bytes) {
+  if (g_counting) count_access(2, src, bytes, 1);
+  std::memcpy(dst, src, bytes);
+}
 
 }  // namespace emu
 
@@ -223,9 +306,14 @@ cudaError_t emuMalloc(void** p, size_t bytes) {
   if (posix_memalign(&q, 256, bytes ? bytes : 1) != 0) { *p = nullptr; return cudaErrorMemoryAllocation; }
   std::memset(q, 0xCD, bytes);        // fresh device memory is not zero
   *p = q;
+  emu::note_alloc(q, bytes);
   return cudaSuccess;
 }
-cudaError_t cudaFree(void* p) { std::free(p); return cudaSuccess; }
+cudaError_t cudaFree(void* p) {
+  if (p) emu::note_free(p);
+  std::free(p);
+  return cudaSuccess;
+}
 cudaError_t cudaMemset(void* p, int v, size_t bytes) { std::memset(p, v, bytes); return cudaSuccess; }
 cudaError_t cudaMemsetAsync(void* p, int v, size_t bytes, cudaStream_t st) {
   submit(st, [=] { std::memset(p, v, bytes); });
@@ -305,4 +393,27 @@ cudaError_t cudaGetDriverEntryPoint(const char* name, void** fn, int, cudaDriver
   *fn = nullptr;
   *res = cudaDriverEntryPointSymbolNotFound;
   return cudaSuccess;
+}
+
+// ---- request counting: control (tests/emu/count_requests.py) -----------------------------------------------------------
+extern "C" void emu_count_enable(int on) { emu::g_counting = on != 0; }
+extern "C" void emu_count_layout(unsigned long long n_bytes, unsigned long long oA_bytes, unsigned long long oI_bytes,
+                                 unsigned long long oG_bytes, unsigned long long m_bytes) {
+  emu::g_n_bytes = n_bytes; emu::g_oA = oA_bytes; emu::g_oI = oI_bytes; emu::g_oG = oG_bytes; emu::g_m_bytes = m_bytes;
+}
+extern "C" void emu_count_reset() { std::lock_guard<std::mutex> lk(emu::g_count_mutex); emu::g_totals.clear(); emu::g_regions.clear(); }
+extern "C" void emu_count_region(const char* name, const void* p, unsigned long long bytes) {
+  std::lock_guard<std::mutex> lk(emu::g_count_mutex);
+  emu::g_regions.push_back(emu::Region{reinterpret_cast<uintptr_t>(p), reinterpret_cast<uintptr_t>(p) + bytes, name});
+}
+// "kind class instructions lanes lines sectors" per line
+extern "C" int emu_count_report(char* out, int cap) {
+  std::lock_guard<std::mutex> lk(emu::g_count_mutex);
+  std::string s;
+  for (auto& [k, t] : emu::g_totals)
+    s += std::to_string(k.first) + " " + k.second + " " + std::to_string(t.instr) + " " + std::to_string(t.lanes) + " " +
+         std::to_string(t.lines) + " " + std::to_string(t.sectors) + "\n";
+  if ((int)s.size() + 1 > cap) return -(int)s.size() - 1;
+  std::memcpy(out, s.c_str(), s.size() + 1);
+  return (int)s.size();
 }
